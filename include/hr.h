@@ -1,0 +1,173 @@
+/*
+ * hr.h -- C ABI of the B200-native hyperbolic-relaxation hot path (arxiv 2501.14030).
+ *
+ * The library advances the (u, v) relaxation system of PAPER.md Sec. 2, Eq. 5
+ *     d_t u = v - eta u
+ *     d_t v = c^2 [ lap u + (1/8) A~_ij A~^ij (psi_singular + u)^-7 ]
+ * by the method-of-lines loop of PAPER.md Alg. 1 l.12-16: RHS -> BC -> RK,
+ * four times per RK4 step, and evaluates the residual of Eq. 4 (Alg. 1 l.9-11).
+ * Everything the paper defers to its references is fixed by the readings C1-C23 in DESIGN.md.
+ *
+ * Conventions
+ *   - Every entry point returns hr_status, never throws or aborts, and writes its outputs only
+ *     on HR_OK.  hr_last_error() gives the text of the calling thread's last failure.
+ *   - "device pointer" = CUDA global memory on hr_params.device; "host pointer" = ordinary or
+ *     pinned host memory.  No torch / C++ types cross this boundary.
+ *   - Grid layout (reading C8): interior points N = (N0, N1, N2); NG = fd_order/2 ghost layers
+ *     on every face; T_a = N_a + 2 NG; N_tot = T0 T1 T2; a grid function is N_tot scalars with
+ *     flat index  idx(i0,i1,i2) = i0 + T0 (i1 + T1 i2), i0 fastest.  Scalars are double
+ *     (HR_F64) or float (HR_F32).  Coordinates: x0 in [0,1] (sinh-compactified radius),
+ *     x1 = theta in [0,pi], x2 = phi in [-pi,pi], cell-centred.
+ *   - All work is enqueued on hr_params.stream (a cudaStream_t, may be NULL = legacy default
+ *     stream).  hr_step is asynchronous with respect to the host; the calls
+ *     that return host values synchronise that stream.
+ *   - There is no CPU fallback: without a CUDA device every compute call fails with HR_ERR_CUDA.
+ */
+#ifndef HR_H
+#define HR_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define HR_API __attribute__((visibility("default")))
+#else
+#define HR_API
+#endif
+
+typedef struct hr_solver hr_solver; /* opaque; created and destroyed by the library */
+
+typedef enum {
+  HR_OK = 0,
+  HR_ERR_INVALID_ARG = 1, /* NULL pointer, N2 odd, N_a < NG, m <= 0, eta < 0, cfl <= 0, ...   */
+  HR_ERR_UNSUPPORTED = 2, /* fd_order / coord / dtype not instantiated                        */
+  HR_ERR_WORKSPACE = 3,   /* workspace too small or misaligned (256 B)                        */
+  HR_ERR_CUDA = 4,        /* a CUDA runtime call failed; text in hr_last_error()              */
+  HR_ERR_NUMERIC = 5      /* a puncture coincides with a grid point (non-finite source)       */
+} hr_status;
+
+typedef enum { HR_SINHSPHERICAL = 0, HR_SINHSYMTP = 1 } hr_coord; /* reading C4            */
+typedef enum { HR_F64 = 0, HR_F32 = 1 } hr_dtype;                 /* reading C19           */
+
+/* One Brandt-Bruegmann puncture: bare mass, Cartesian position, Bowen-York
+ * linear momentum P and spin S (readings C1, C2). */
+typedef struct {
+  double m;
+  double pos[3];
+  double P[3];
+  double S[3];
+} hr_puncture;
+
+/* Problem statement: grid, coordinate system, FD order, punctures, eta, CFL (Eq. 4-5
+ * and Alg. 1 l.2-7). */
+typedef struct {
+  int32_t n[3];          /* interior points N0 N1 N2; N2 even; N_a >= NG                      */
+  int32_t coord;         /* hr_coord                                                          */
+  int32_t fd_order;      /* 4, 6, 8, 10 (also 2, 12): centred stencils, NG = fd_order/2 (C7,
+                            C11)                                                */
+  int32_t dtype;         /* hr_dtype: arithmetic and storage type of state and RHS            */
+  double amp, sinhw;     /* AMPL/SINHW (SinhSpherical) or AMAX/SINHWAA (SinhSymTP) (C4, C5)   */
+  double bscale;         /* SinhSymTP focal half-distance b; ignored for SinhSpherical        */
+  double origin[3];      /* Cartesian position of the grid centre (C6)                        */
+  int32_t n_punctures;   /* >= 0                                                              */
+  int32_t residual_mode; /* default mode of hr_residual: 0 volume-weighted RMS, 1 plain RMS
+                            (C16)                                                             */
+  const hr_puncture* punctures; /* host pointer, read during hr_create only (copied)          */
+  double eta;            /* damping factor of Eq. 5 (C10)                        */
+  double cfl;            /* dt = cfl * ds_min over interior points (C9)                       */
+  double c_min;          /* wave-speed normalisation: c(x) = c_min ds(x)/ds_min (C9)          */
+  int32_t device;        /* CUDA device ordinal                                               */
+  int32_t variant;       /* kernel arrangement: 0 = default (fused, tiled);
+                            1 = paper arrangement ablation (one thread per point, direct
+                            global loads, k stored, separate RK kernel)     */
+  void* stream;          /* cudaStream_t owned by the caller; must outlive the solver         */
+} hr_params;
+
+/* Bytes of device workspace hr_create needs for these parameters (10 grid functions, the
+ * (i0,i1) coefficient planes, the boundary lists, reduction scratch). */
+HR_API hr_status hr_workspace_bytes(const hr_params* p, size_t* bytes);
+
+/* Alg. 1 l.2-7: coordinate arrays, reference-metric factor planes, wave speed
+ * and dt (C9), inner/outer boundary containers (C13, C14; integer closed form), then the
+ * one-time device source kernel psi_BL and (1/8) A~_ij A~^ij (C1, C2), and u = v = 0 (C17).
+ * workspace_dev: device pointer, 256-byte aligned, >= hr_workspace_bytes; owned by the caller,
+ * must outlive the solver; the library never frees it.  *out receives the handle. */
+HR_API hr_status hr_create(const hr_params* p, void* workspace_dev, size_t workspace_bytes,
+                    hr_solver** out);
+
+/* Releases the handle and its host metadata / CUDA graph.  NULL is accepted. */
+HR_API hr_status hr_destroy(hr_solver* s);
+
+/* Alg. 1 l.12-16 x n_steps: n_steps classic RK4 steps (C15), each four substeps of
+ * [fused RHS (Eq. 5) + radiation condition at the outer points (C13) + RK combine] followed by the
+ * inner-boundary fill (C14).  Enqueues on the stream and returns; n_steps >= 0. */
+HR_API hr_status hr_step(hr_solver* s, int64_t n_steps);
+
+/* Alg. 1 l.9-11: H = lap u + S (psi_BL + u)^-7 at interior points and its grid L2 norm in the
+ * solver's residual_mode (C16), accumulated in fp64 with a fixed reduction order.
+ * *out (host pointer) receives the norm; synchronises the stream. */
+HR_API hr_status hr_residual(hr_solver* s, double* out);
+/* Same with an explicit mode (0 or 1); out3 (host pointer, 3 doubles) receives
+ * { norm, sum w H^2, sum w }. */
+HR_API hr_status hr_residual_ex(hr_solver* s, int32_t mode, double* out3);
+/* Asynchronous form for the relaxation loop (Alg. 1 l.9-11 inside the time loop): enqueues the
+ * H kernel and the reduction and writes { sum w H^2, sum w } (2 doubles) to out2_dev (device
+ * pointer); no host synchronisation. */
+HR_API hr_status hr_residual_async(hr_solver* s, int32_t mode, double* out2_dev);
+
+/* Copy the current u (or v), N_tot scalars of the solver's dtype in the layout above, ghost
+ * points included, to dst (device pointer if dst_on_device != 0, else host pointer).
+ * bytes must equal N_tot * sizeof(scalar).  Synchronises the stream. */
+HR_API hr_status hr_get_u(hr_solver* s, void* dst, size_t bytes, int32_t dst_on_device);
+HR_API hr_status hr_get_v(hr_solver* s, void* dst, size_t bytes, int32_t dst_on_device);
+
+/* ---- hooks for the parity contract (a production user does not need these) ---- */
+
+/* Replace the state by N_tot scalars each of u and v (solver dtype, layout above).  The inner
+ * ghost entries are then overwritten by their sources (C14/C15: ghosts mirror sources). */
+HR_API hr_status hr_set_state(hr_solver* s, const void* u, const void* v, int32_t src_on_device);
+
+/* One evaluation of Alg. 1 l.13-14 on the current state: k = RHS at interior points, radiation
+ * condition at outer points, inner fill; N_tot scalars each into the device pointers ku_dev,
+ * kv_dev.  Uses the same device arithmetic as hr_step's fused kernels. */
+HR_API hr_status hr_eval_rhs(hr_solver* s, void* ku_dev, void* kv_dev);
+
+/* Copies of the constant source terms psi_BL and S = (1/8) A~_ij A~^ij (solver dtype, N_tot
+ * each) to host pointers (either may be NULL). */
+HR_API hr_status hr_get_source(hr_solver* s, void* psi_host, void* S_host);
+
+/* Boundary containers (C13, C14), ascending destination index.  With NULL arrays only the counts
+ * are returned.  Host pointers. */
+HR_API hr_status hr_get_bc_lists(hr_solver* s, int32_t* inner_dst, int32_t* inner_src, int64_t* n_inner,
+                          int32_t* outer_idx, int64_t* n_outer);
+
+/* dt and ds_min (C9), NG, T[3], N_tot.  Any pointer may be NULL. */
+HR_API hr_status hr_get_info(hr_solver* s, double* dt, double* dsmin, int32_t* nghosts, int32_t* T,
+                      int64_t* total_pts);
+
+/* Host-only (no CUDA call, works without a device): the tables hr_create builds on the host
+ * for these parameters -- Alg. 1 l.2-4.  All outputs are host pointers and optional (NULL):
+ * dt, ds_min (C9); the boundary containers (C13, C14) with their counts; planes7 = 7 x T0*T1
+ * doubles { g00/dx0^2, g11/dx1^2, g22/dx2^2, g0/dx0, g1/dx1, c^2, |h0 h1 h2| }, index i0 + T0 i1;
+ * outer3 = 3 x NG*T1 doubles { c rad0/(2 dx0), c rad1/(2 dx1), c/r }, index (i0-N0-NG) + NG i1. */
+HR_API hr_status hr_host_setup(const hr_params* p, double* dt, double* dsmin, int64_t* n_inner,
+                               int64_t* n_outer, int32_t* inner_dst, int32_t* inner_src,
+                               int32_t* outer_idx, double* planes7, double* outer3);
+
+/* Number of kernel launches one hr_step(1) enqueues (for bench.py's gpu_launches). */
+HR_API hr_status hr_launches_per_step(hr_solver* s, int32_t* n);
+
+/* Thread-local, static storage; never NULL. */
+HR_API const char* hr_last_error(void);
+
+/* Library version string, e.g. "hr-b200 0.1 (sm_100a)". */
+HR_API const char* hr_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HR_H */

@@ -1,0 +1,644 @@
+// hr_api.cu -- the extern "C" boundary of include/hr.h and the host-side set-up
+// (Alg. 1 l.2-7).  Host logic only: coordinate tables, reference-metric
+// factor planes, wave speed / dt, the closed-form integer boundary maps, workspace carving,
+// CUDA-graph capture of one RK4 step.  Every per-point operation of the hot path runs in
+// hr_kernels.cu; there is no CPU fallback.  Product code: nothing here touches oracle/.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <limits>
+#include <new>
+
+#include "hr_internal.h"
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+hr_status fail(hr_status st, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+  return st;
+}
+
+#define HR_CUDA(call)                                                                       \
+  do {                                                                                      \
+    cudaError_t e__ = (call);                                                               \
+    if (e__ != cudaSuccess)                                                                 \
+      return fail(HR_ERR_CUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e__),     \
+                  __FILE__, __LINE__);                                                      \
+  } while (0)
+
+#define HR_TRY(expr)                \
+  do {                              \
+    hr_status st__ = (expr);        \
+    if (st__ != HR_OK) return st__; \
+  } while (0)
+
+constexpr double kPi = 3.141592653589793238462643383279502884;
+
+size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+hr_status validate(const hr_params* p) {
+  if (!p) return fail(HR_ERR_INVALID_ARG, "params is NULL");
+  if (p->fd_order % 2 != 0 || p->fd_order < 2 || p->fd_order > 2 * HR_MAX_NG)
+    return fail(HR_ERR_UNSUPPORTED, "fd_order %d not in {2,4,...,%d}", p->fd_order, 2 * HR_MAX_NG);
+  if (p->coord != HR_SINHSPHERICAL && p->coord != HR_SINHSYMTP)
+    return fail(HR_ERR_UNSUPPORTED, "coord %d unknown", p->coord);
+  if (p->dtype != HR_F64 && p->dtype != HR_F32)
+    return fail(HR_ERR_UNSUPPORTED, "dtype %d unknown", p->dtype);
+  if (p->variant != 0) return fail(HR_ERR_UNSUPPORTED, "variant %d unknown", p->variant);
+  const int ng = p->fd_order / 2;
+  for (int a = 0; a < 3; ++a)
+    if (p->n[a] < ng)
+      return fail(HR_ERR_INVALID_ARG, "n[%d] = %d is smaller than NG = %d", a, p->n[a], ng);
+  if (p->n[2] % 2) return fail(HR_ERR_INVALID_ARG, "n[2] = %d must be even (C14)", p->n[2]);
+  const double tot = double(p->n[0] + 2 * ng) * double(p->n[1] + 2 * ng) * double(p->n[2] + 2 * ng);
+  if (tot >= 2147483647.0) return fail(HR_ERR_INVALID_ARG, "grid exceeds int32 index range");
+  if (!(p->amp > 0) || !(p->sinhw > 0)) return fail(HR_ERR_INVALID_ARG, "amp, sinhw must be > 0");
+  if (p->coord == HR_SINHSYMTP && !(p->bscale > 0))
+    return fail(HR_ERR_INVALID_ARG, "bscale must be > 0 for SinhSymTP");
+  if (!(p->cfl > 0) || !(p->c_min > 0) || !(p->eta >= 0))
+    return fail(HR_ERR_INVALID_ARG, "need cfl > 0, c_min > 0, eta >= 0");
+  if (p->residual_mode != 0 && p->residual_mode != 1)
+    return fail(HR_ERR_INVALID_ARG, "residual_mode must be 0 or 1");
+  if (p->n_punctures < 0 || (p->n_punctures > 0 && !p->punctures))
+    return fail(HR_ERR_INVALID_ARG, "bad puncture list");
+  for (int q = 0; q < p->n_punctures; ++q)
+    if (!(p->punctures[q].m > 0)) return fail(HR_ERR_INVALID_ARG, "puncture %d: m must be > 0", q);
+  return HR_OK;
+}
+
+// Workspace carving shared by hr_workspace_bytes and hr_create.
+struct Layout {
+  size_t off_field[10];
+  size_t off_plane[6];
+  size_t off_rad[3];
+  size_t off_wvol, off_inner_dst, off_inner_src, off_partials, off_result;
+  size_t off_rho, off_rhoz, off_sinth, off_costh, off_sinph, off_cosph, off_punct;
+  size_t total;
+  int64_t ntot, n_inner;
+  int T[3], ng;
+  int nblocks;
+};
+
+Layout make_layout(const hr_params* p) {
+  Layout L{};
+  L.ng = p->fd_order / 2;
+  for (int a = 0; a < 3; ++a) L.T[a] = p->n[a] + 2 * L.ng;
+  L.ntot = (int64_t)L.T[0] * L.T[1] * L.T[2];
+  L.n_inner = L.ntot - (int64_t)p->n[0] * p->n[1] * p->n[2] - (int64_t)L.ng * p->n[1] * p->n[2];
+  const size_t w = p->dtype == HR_F64 ? 8 : 4;
+  size_t off = 0;
+  auto take = [&](size_t bytes) {
+    size_t o = off;
+    off = align_up(off + bytes);
+    return o;
+  };
+  for (int f = 0; f < 10; ++f) L.off_field[f] = take((size_t)L.ntot * w);
+  const size_t np = (size_t)L.T[0] * L.T[1];
+  for (int f = 0; f < 6; ++f) L.off_plane[f] = take(np * w);
+  for (int f = 0; f < 3; ++f) L.off_rad[f] = take((size_t)L.ng * L.T[1] * w);
+  L.off_wvol = take(np * 8);
+  L.off_inner_dst = take((size_t)L.n_inner * 4 + 4);
+  L.off_inner_src = take((size_t)L.n_inner * 4 + 4);
+  HrGrid g{};
+  g.n0 = p->n[0];
+  g.n1 = p->n[1];
+  g.n2 = p->n[2];
+  L.nblocks = hrk_residual_blocks(g);
+  L.off_partials = take((size_t)L.nblocks * 16);
+  L.off_result = take(64);
+  L.off_rho = take((size_t)L.T[0] * 8);
+  L.off_rhoz = take((size_t)L.T[0] * 8);
+  L.off_sinth = take((size_t)L.T[1] * 8);
+  L.off_costh = take((size_t)L.T[1] * 8);
+  L.off_sinph = take((size_t)L.T[2] * 8);
+  L.off_cosph = take((size_t)L.T[2] * 8);
+  L.off_punct = take((size_t)(p->n_punctures + 1) * 80);
+  L.total = off;
+  return L;
+}
+
+// Reference-metric quantities at one (x0, theta) (reading C4 for the factors of
+//   lap u = g00 u_00 + g11 u_11 + g22 u_22 + g0 u_0 + g1 u_1,
+// C9 for the proper spacings, C13 for the radial-derivative factors).
+struct MetricPoint {
+  double g00, g11, g22, g0, g1;
+  double h0, h1, h2;
+  double rad0, rad1, invr;
+};
+
+struct Radial {  // rho(x0) = AMP sinh(x0/W)/sinh(1/W) and derivatives
+  double f, d1, d2;
+};
+
+Radial radial_map(const hr_params& p, double x0) {
+  const double inv = 1.0 / std::sinh(1.0 / p.sinhw);
+  Radial r;
+  r.f = p.amp * std::sinh(x0 / p.sinhw) * inv;
+  r.d1 = p.amp * std::cosh(x0 / p.sinhw) * inv / p.sinhw;
+  r.d2 = r.f / (p.sinhw * p.sinhw);
+  return r;
+}
+
+MetricPoint metric_point(const hr_params& p, const Radial& R, double sth, double cth) {
+  MetricPoint m;
+  const double A = R.f, A1 = R.d1, A2 = R.d2;
+  if (p.coord == HR_SINHSPHERICAL) {
+    // flat metric in spherical coordinates with r = rho(x0)
+    m.h0 = A1;
+    m.h1 = A;
+    m.h2 = A * sth;
+    m.g00 = 1.0 / (A1 * A1);
+    m.g11 = 1.0 / (A * A);
+    m.g22 = m.g11 / (sth * sth);
+    m.g0 = (2.0 / A - A2 / (A1 * A1)) / A1;
+    m.g1 = m.g11 * cth / sth;
+    m.rad0 = 1.0 / A1;
+    m.rad1 = 0.0;
+    m.invr = 1.0 / A;
+  } else {
+    // prolate-spheroidal-like (foci at z = +-b): Sigma = A^2 + b^2 sin^2, AB = A^2 + b^2
+    const double b2 = p.bscale * p.bscale;
+    const double AB = A * A + b2;
+    const double Sig = A * A + b2 * sth * sth;
+    const double iSig = 1.0 / Sig;
+    m.h0 = A1 * std::sqrt(Sig / AB);
+    m.h1 = std::sqrt(Sig);
+    m.h2 = A * sth;
+    m.g00 = AB * iSig / (A1 * A1);
+    m.g11 = iSig;
+    m.g22 = 1.0 / (A * A * sth * sth);
+    m.g0 = iSig * ((2.0 * A * A + b2) / (A * A1) - AB * A2 / (A1 * A1 * A1));
+    m.g1 = iSig * cth / sth;
+    const double r = std::sqrt(A * A + b2 * cth * cth);  // distance from the grid centre
+    m.rad0 = A * AB / (A1 * r * Sig);
+    m.rad1 = -b2 * sth * cth / (r * Sig);
+    m.invr = 1.0 / r;
+  }
+  return m;
+}
+
+// Closed-form integer inner map (reading C14).  Returns the source index triple of ghost point
+// (i0,i1,i2); the caller has already excluded interior and outer points.
+inline void inner_source(const hr_params& p, int ng, const int T[3], int i0, int i1, int i2,
+                         int& j0, int& j1, int& j2) {
+  const int N1 = p.n[1], N2 = p.n[2];
+  int flips = 0;
+  j0 = i0;
+  j1 = i1;
+  if (i0 < ng) {  // x0 -> -x0 : rho -> -rho
+    j0 = 2 * ng - 1 - i0;
+    ++flips;
+    if (p.coord == HR_SINHSPHERICAL) j1 = T[1] - 1 - j1;  // r -> -r also sends theta -> pi - theta
+  }
+  if (j1 < ng) {  // theta -> -theta
+    j1 = 2 * ng - 1 - j1;
+    ++flips;
+  } else if (j1 >= N1 + ng) {  // theta -> 2 pi - theta
+    j1 = 2 * (N1 + ng) - 1 - j1;
+    ++flips;
+  }
+  int k = i2 - ng + (flips & 1) * (N2 / 2);  // each flip shifts phi by pi
+  k %= N2;
+  if (k < 0) k += N2;
+  j2 = k + ng;
+}
+
+template <typename T>
+void to_working(const std::vector<double>& src, std::vector<char>& dst) {
+  dst.resize(src.size() * sizeof(T));
+  T* d = reinterpret_cast<T*>(dst.data());
+  for (size_t i = 0; i < src.size(); ++i) d[i] = (T)src[i];  // setup in fp64, rounded once (C19)
+}
+
+hr_status upload(void* dst, const void* src, size_t bytes, cudaStream_t st) {
+  if (bytes == 0) return HR_OK;
+  HR_CUDA(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, st));
+  HR_CUDA(cudaStreamSynchronize(st));  // src is pageable and about to be freed
+  return HR_OK;
+}
+
+hr_status upload_plane(const hr_solver* s, void* dst, const std::vector<double>& v) {
+  std::vector<char> tmp;
+  if (s->p.dtype == HR_F64)
+    to_working<double>(v, tmp);
+  else
+    to_working<float>(v, tmp);
+  return upload(dst, tmp.data(), tmp.size(), s->stream);
+}
+
+// Everything hr_create computes on the host (Alg. 1 l.2-4) before touching the device.
+struct HostSetup {
+  int ng, T[3];
+  double dx[3], dsmin, dt;
+  std::vector<double> rho, rhoz, sth, cth, sph, cph;           // 1-D coordinate tables
+  std::vector<double> l00, l11, l22, l0, l1, c2, wv;           // (i0,i1) planes
+  std::vector<double> r0, r1, ri;                              // compact outer planes (ng x T1)
+  std::vector<int32_t> inner_dst, inner_src, outer_idx;
+};
+
+hr_status host_setup(const hr_params* p, HostSetup& H) {
+  const int ng = H.ng = p->fd_order / 2;
+  for (int a = 0; a < 3; ++a) H.T[a] = p->n[a] + 2 * ng;
+  const int T0 = H.T[0], T1 = H.T[1], T2 = H.T[2];
+  const int n0 = p->n[0], n1 = p->n[1], n2 = p->n[2];
+  // ---- Alg. 1 l.2: cell-centred coordinate tables (C8) ----
+  H.dx[0] = 1.0 / n0;
+  H.dx[1] = kPi / n1;
+  H.dx[2] = 2.0 * kPi / n2;
+  std::vector<Radial> R(T0);
+  H.rho.resize(T0); H.rhoz.resize(T0); H.sth.resize(T1); H.cth.resize(T1); H.sph.resize(T2);
+  H.cph.resize(T2);
+  for (int i = 0; i < T0; ++i) {
+    R[i] = radial_map(*p, (i - ng + 0.5) * H.dx[0]);
+    H.rho[i] = R[i].f;
+    H.rhoz[i] =
+        p->coord == HR_SINHSYMTP ? std::sqrt(R[i].f * R[i].f + p->bscale * p->bscale) : R[i].f;
+  }
+  for (int i = 0; i < T1; ++i) {
+    const double th = (i - ng + 0.5) * H.dx[1];
+    H.sth[i] = std::sin(th);
+    H.cth[i] = std::cos(th);
+  }
+  for (int i = 0; i < T2; ++i) {
+    const double ph = -kPi + (i - ng + 0.5) * H.dx[2];
+    H.sph[i] = std::sin(ph);
+    H.cph[i] = std::cos(ph);
+  }
+
+  // ---- Alg. 1 l.3: reference-metric factor planes, wave speed, dt (C4, C9, C13, C16) ----
+  const size_t np = (size_t)T0 * T1;
+  for (auto* v : {&H.l00, &H.l11, &H.l22, &H.l0, &H.l1, &H.c2, &H.wv}) v->resize(np);
+  std::vector<double> ds(np);
+  std::vector<MetricPoint> mp(np);
+  double dsmin = std::numeric_limits<double>::infinity();
+  for (int i1 = 0; i1 < T1; ++i1)
+    for (int i0 = 0; i0 < T0; ++i0) {
+      const size_t q = (size_t)i0 + (size_t)T0 * i1;
+      const MetricPoint m = metric_point(*p, R[i0], H.sth[i1], H.cth[i1]);
+      mp[q] = m;
+      const double d = std::fmin(std::fabs(m.h0) * H.dx[0],
+                                 std::fmin(std::fabs(m.h1) * H.dx[1], std::fabs(m.h2) * H.dx[2]));
+      ds[q] = d;
+      H.wv[q] = std::fabs(m.h0 * m.h1 * m.h2);
+      const bool interior = i0 >= ng && i0 < n0 + ng && i1 >= ng && i1 < n1 + ng;
+      if (interior && d < dsmin) dsmin = d;
+    }
+  H.dsmin = dsmin;
+  H.dt = p->cfl * dsmin;
+  H.r0.assign((size_t)ng * T1, 0.0);
+  H.r1.assign((size_t)ng * T1, 0.0);
+  H.ri.assign((size_t)ng * T1, 0.0);
+  for (int i1 = 0; i1 < T1; ++i1)
+    for (int i0 = 0; i0 < T0; ++i0) {
+      const size_t q = (size_t)i0 + (size_t)T0 * i1;
+      const MetricPoint& m = mp[q];
+      const double c = p->c_min * ds[q] / dsmin;
+      H.l00[q] = m.g00 / (H.dx[0] * H.dx[0]);
+      H.l11[q] = m.g11 / (H.dx[1] * H.dx[1]);
+      H.l22[q] = m.g22 / (H.dx[2] * H.dx[2]);
+      H.l0[q] = m.g0 / H.dx[0];
+      H.l1[q] = m.g1 / H.dx[1];
+      H.c2[q] = c * c;
+      if (i0 >= n0 + ng) {
+        const size_t qo = (size_t)(i0 - (n0 + ng)) + (size_t)ng * i1;
+        H.r0[qo] = c * m.rad0 / (2.0 * H.dx[0]);
+        H.r1[qo] = c * m.rad1 / (2.0 * H.dx[1]);
+        H.ri[qo] = c * m.invr;
+      }
+    }
+
+  // ---- Alg. 1 l.4: boundary containers (C13, C14), ascending destination index ----
+  const int64_t ntot = (int64_t)T0 * T1 * T2;
+  const int64_t n_outer = (int64_t)ng * n1 * n2;
+  const int64_t n_inner = ntot - (int64_t)n0 * n1 * n2 - n_outer;
+  H.inner_dst.reserve((size_t)n_inner);
+  H.inner_src.reserve((size_t)n_inner);
+  H.outer_idx.reserve((size_t)n_outer);
+  for (int i2 = 0; i2 < T2; ++i2)
+    for (int i1 = 0; i1 < T1; ++i1) {
+      const bool in12 = i1 >= ng && i1 < n1 + ng && i2 >= ng && i2 < n2 + ng;
+      for (int i0 = 0; i0 < T0; ++i0) {
+        if (in12 && i0 >= ng) {
+          if (i0 >= n0 + ng) H.outer_idx.push_back(i0 + T0 * (i1 + T1 * i2));
+          continue;  // interior or outer
+        }
+        int j0, j1, j2;
+        inner_source(*p, ng, H.T, i0, i1, i2, j0, j1, j2);
+        H.inner_dst.push_back(i0 + T0 * (i1 + T1 * i2));
+        H.inner_src.push_back(j0 + T0 * (j1 + T1 * j2));
+      }
+    }
+  if ((int64_t)H.inner_dst.size() != n_inner || (int64_t)H.outer_idx.size() != n_outer)
+    return fail(HR_ERR_INVALID_ARG, "internal: boundary list sizes inconsistent");
+  return HR_OK;
+}
+
+hr_status enqueue_rk4_step(const hr_solver* s) {
+  for (int stage = 1; stage <= 4; ++stage) HR_CUDA(hrk_substep(s, stage));
+  return HR_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* hr_last_error(void) { return g_err; }
+
+const char* hr_version(void) { return "hr-b200 0.1 (sm_100a)"; }
+
+hr_status hr_workspace_bytes(const hr_params* p, size_t* bytes) {
+  hr_status st = validate(p);
+  if (st != HR_OK) return st;
+  if (!bytes) return fail(HR_ERR_INVALID_ARG, "bytes is NULL");
+  *bytes = make_layout(p).total;
+  return HR_OK;
+}
+
+hr_status hr_create(const hr_params* p, void* workspace_dev, size_t workspace_bytes,
+                    hr_solver** out) {
+  hr_status st = validate(p);
+  if (st != HR_OK) return st;
+  if (!out) return fail(HR_ERR_INVALID_ARG, "out is NULL");
+  const Layout L = make_layout(p);
+  if (!workspace_dev || (reinterpret_cast<uintptr_t>(workspace_dev) & 255u))
+    return fail(HR_ERR_WORKSPACE, "workspace must be a 256-byte aligned device pointer");
+  if (workspace_bytes < L.total)
+    return fail(HR_ERR_WORKSPACE, "workspace has %zu bytes, %zu needed", workspace_bytes, L.total);
+  HR_CUDA(cudaSetDevice(p->device));
+
+  hr_solver* s = new (std::nothrow) hr_solver();
+  if (!s) return fail(HR_ERR_INVALID_ARG, "out of host memory");
+  struct Guard {
+    hr_solver* s;
+    ~Guard() { if (s) hr_destroy(s); }
+  } guard{s};
+
+  s->p = *p;
+  s->punctures.assign(p->punctures, p->punctures + p->n_punctures);
+  s->p.punctures = s->punctures.data();
+  s->stream = static_cast<cudaStream_t>(p->stream);
+  s->step_graph = nullptr;
+  s->workspace = workspace_dev;
+  s->workspace_bytes = workspace_bytes;
+  s->scalar_bytes = p->dtype == HR_F64 ? 8 : 4;
+  const int ng = L.ng;
+  HrGrid& g = s->g;
+  g.n0 = p->n[0]; g.n1 = p->n[1]; g.n2 = p->n[2];
+  g.ng = ng;
+  g.T0 = L.T[0]; g.T1 = L.T[1]; g.T2 = L.T[2];
+  g.s1 = g.T0;
+  g.s2 = (int64_t)g.T0 * g.T1;
+  g.ntot = L.ntot;
+  g.n_inner = L.n_inner;
+  g.n_outer_cols = ng;
+  s->n_outer = (int64_t)ng * g.n1 * g.n2;
+  s->max_partials = L.nblocks;
+
+  char* base = static_cast<char*>(workspace_dev);
+  HrArrays& a = s->a;
+  a.Y[0] = base + L.off_field[0];   a.Y[1] = base + L.off_field[1];
+  a.A[0] = base + L.off_field[2];   a.A[1] = base + L.off_field[3];
+  a.B[0] = base + L.off_field[4];   a.B[1] = base + L.off_field[5];
+  a.ACC[0] = base + L.off_field[6]; a.ACC[1] = base + L.off_field[7];
+  a.psi = base + L.off_field[8];    a.S = base + L.off_field[9];
+  a.L00 = base + L.off_plane[0]; a.L11 = base + L.off_plane[1]; a.L22 = base + L.off_plane[2];
+  a.L0 = base + L.off_plane[3];  a.L1 = base + L.off_plane[4];  a.C2 = base + L.off_plane[5];
+  a.RAD0 = base + L.off_rad[0]; a.RAD1 = base + L.off_rad[1]; a.RADI = base + L.off_rad[2];
+  a.Wvol = reinterpret_cast<double*>(base + L.off_wvol);
+  a.inner_dst = reinterpret_cast<int32_t*>(base + L.off_inner_dst);
+  a.inner_src = reinterpret_cast<int32_t*>(base + L.off_inner_src);
+  a.partials = reinterpret_cast<double*>(base + L.off_partials);
+  a.result2 = reinterpret_cast<double*>(base + L.off_result);
+  a.rho = reinterpret_cast<double*>(base + L.off_rho);
+  a.rhoz = reinterpret_cast<double*>(base + L.off_rhoz);
+  a.sinth = reinterpret_cast<double*>(base + L.off_sinth);
+  a.costh = reinterpret_cast<double*>(base + L.off_costh);
+  a.sinph = reinterpret_cast<double*>(base + L.off_sinph);
+  a.cosph = reinterpret_cast<double*>(base + L.off_cosph);
+  a.punct = reinterpret_cast<double*>(base + L.off_punct);
+
+  // ---- Alg. 1 l.2-4 on the host ----
+  HostSetup H;
+  HR_TRY(host_setup(p, H));
+  for (int a = 0; a < 3; ++a) s->dx[a] = H.dx[a];
+  s->dsmin = H.dsmin;
+  s->dt = H.dt;
+  s->inner_dst = std::move(H.inner_dst);
+  s->inner_src = std::move(H.inner_src);
+  s->outer_idx = std::move(H.outer_idx);
+  const size_t np = (size_t)g.T0 * g.T1;
+
+  // ---- upload tables ----
+  HR_TRY(upload_plane(s, a.L00, H.l00));
+  HR_TRY(upload_plane(s, a.L11, H.l11));
+  HR_TRY(upload_plane(s, a.L22, H.l22));
+  HR_TRY(upload_plane(s, a.L0, H.l0));
+  HR_TRY(upload_plane(s, a.L1, H.l1));
+  HR_TRY(upload_plane(s, a.C2, H.c2));
+  HR_TRY(upload_plane(s, a.RAD0, H.r0));
+  HR_TRY(upload_plane(s, a.RAD1, H.r1));
+  HR_TRY(upload_plane(s, a.RADI, H.ri));
+  HR_TRY(upload(a.Wvol, H.wv.data(), np * 8, s->stream));
+  HR_TRY(upload(a.inner_dst, s->inner_dst.data(), s->inner_dst.size() * 4, s->stream));
+  HR_TRY(upload(a.inner_src, s->inner_src.data(), s->inner_src.size() * 4, s->stream));
+  HR_TRY(upload(a.rho, H.rho.data(), H.rho.size() * 8, s->stream));
+  HR_TRY(upload(a.rhoz, H.rhoz.data(), H.rhoz.size() * 8, s->stream));
+  HR_TRY(upload(a.sinth, H.sth.data(), H.sth.size() * 8, s->stream));
+  HR_TRY(upload(a.costh, H.cth.data(), H.cth.size() * 8, s->stream));
+  HR_TRY(upload(a.sinph, H.sph.data(), H.sph.size() * 8, s->stream));
+  HR_TRY(upload(a.cosph, H.cph.data(), H.cph.size() * 8, s->stream));
+  static_assert(sizeof(hr_puncture) == 80, "hr_puncture is 10 packed doubles");
+  HR_TRY(upload(a.punct, s->punctures.data(), s->punctures.size() * sizeof(hr_puncture), s->stream));
+
+  // ---- Alg. 1 l.5, 7: zero state (C17) and constant source terms on the device ----
+  const size_t fb = (size_t)g.ntot * s->scalar_bytes;
+  for (void* f : {a.Y[0], a.Y[1], a.A[0], a.A[1], a.B[0], a.B[1], a.ACC[0], a.ACC[1]})
+    HR_CUDA(cudaMemsetAsync(f, 0, fb, s->stream));
+  HR_CUDA(hrk_source(s));
+  int bad = 0;
+  HR_CUDA(cudaMemcpyAsync(&bad, a.result2, sizeof(int), cudaMemcpyDeviceToHost, s->stream));
+  HR_CUDA(cudaStreamSynchronize(s->stream));
+  if (bad) return fail(HR_ERR_NUMERIC, "a puncture coincides with a grid point");
+
+  // ---- one RK4 step as a CUDA graph (launch-bound on small grids) ----
+  s->launches_per_step = 4 * hrk_launches_per_substep(s);
+  if (s->stream != nullptr) {
+    cudaGraph_t graph = nullptr;
+    if (cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+      hr_status cst = enqueue_rk4_step(s);
+      cudaError_t ce = cudaStreamEndCapture(s->stream, &graph);
+      if (cst == HR_OK && ce == cudaSuccess && graph) {
+        if (cudaGraphInstantiate(&s->step_graph, graph, 0) != cudaSuccess) s->step_graph = nullptr;
+      }
+      if (graph) cudaGraphDestroy(graph);
+    }
+    cudaGetLastError();  // a failed capture falls back to direct launches of the same kernels
+  }
+
+  guard.s = nullptr;
+  *out = s;
+  return HR_OK;
+}
+
+hr_status hr_host_setup(const hr_params* p, double* dt, double* dsmin, int64_t* n_inner,
+                        int64_t* n_outer, int32_t* inner_dst, int32_t* inner_src,
+                        int32_t* outer_idx, double* planes7, double* outer3) {
+  hr_status st = validate(p);
+  if (st != HR_OK) return st;
+  HostSetup H;
+  HR_TRY(host_setup(p, H));
+  if (dt) *dt = H.dt;
+  if (dsmin) *dsmin = H.dsmin;
+  if (n_inner) *n_inner = (int64_t)H.inner_dst.size();
+  if (n_outer) *n_outer = (int64_t)H.outer_idx.size();
+  if (inner_dst) memcpy(inner_dst, H.inner_dst.data(), H.inner_dst.size() * 4);
+  if (inner_src) memcpy(inner_src, H.inner_src.data(), H.inner_src.size() * 4);
+  if (outer_idx) memcpy(outer_idx, H.outer_idx.data(), H.outer_idx.size() * 4);
+  if (planes7) {
+    const size_t np = H.l00.size();
+    const std::vector<double>* v[7] = {&H.l00, &H.l11, &H.l22, &H.l0, &H.l1, &H.c2, &H.wv};
+    for (int f = 0; f < 7; ++f) memcpy(planes7 + f * np, v[f]->data(), np * 8);
+  }
+  if (outer3) {
+    const size_t no = H.r0.size();
+    memcpy(outer3, H.r0.data(), no * 8);
+    memcpy(outer3 + no, H.r1.data(), no * 8);
+    memcpy(outer3 + 2 * no, H.ri.data(), no * 8);
+  }
+  return HR_OK;
+}
+
+hr_status hr_destroy(hr_solver* s) {
+  if (!s) return HR_OK;
+  if (s->step_graph) cudaGraphExecDestroy(s->step_graph);
+  delete s;
+  return HR_OK;
+}
+
+hr_status hr_step(hr_solver* s, int64_t n_steps) {
+  if (!s) return fail(HR_ERR_INVALID_ARG, "solver is NULL");
+  if (n_steps < 0) return fail(HR_ERR_INVALID_ARG, "n_steps < 0");
+  for (int64_t i = 0; i < n_steps; ++i) {
+    if (s->step_graph) {
+      HR_CUDA(cudaGraphLaunch(s->step_graph, s->stream));
+    } else {
+      hr_status st = enqueue_rk4_step(s);
+      if (st != HR_OK) return st;
+    }
+  }
+  return HR_OK;
+}
+
+hr_status hr_residual_async(hr_solver* s, int32_t mode, double* out2_dev) {
+  if (!s || !out2_dev) return fail(HR_ERR_INVALID_ARG, "NULL argument");
+  if (mode != 0 && mode != 1) return fail(HR_ERR_INVALID_ARG, "mode must be 0 or 1");
+  HR_CUDA(hrk_residual(s, mode, out2_dev));
+  return HR_OK;
+}
+
+hr_status hr_residual_ex(hr_solver* s, int32_t mode, double* out3) {
+  if (!s || !out3) return fail(HR_ERR_INVALID_ARG, "NULL argument");
+  hr_status st = hr_residual_async(s, mode, s->a.result2);
+  if (st != HR_OK) return st;
+  double h[2];
+  HR_CUDA(cudaMemcpyAsync(h, s->a.result2, sizeof(h), cudaMemcpyDeviceToHost, s->stream));
+  HR_CUDA(cudaStreamSynchronize(s->stream));
+  out3[0] = std::sqrt(h[0] / h[1]);
+  out3[1] = h[0];
+  out3[2] = h[1];
+  return HR_OK;
+}
+
+hr_status hr_residual(hr_solver* s, double* out) {
+  if (!s || !out) return fail(HR_ERR_INVALID_ARG, "NULL argument");
+  double o3[3];
+  hr_status st = hr_residual_ex(s, s->p.residual_mode, o3);
+  if (st == HR_OK) *out = o3[0];
+  return st;
+}
+
+static hr_status get_field(hr_solver* s, const void* src, void* dst, size_t bytes, int on_device) {
+  if (!s || !dst) return fail(HR_ERR_INVALID_ARG, "NULL argument");
+  const size_t need = (size_t)s->g.ntot * s->scalar_bytes;
+  if (bytes != need) return fail(HR_ERR_INVALID_ARG, "bytes = %zu, expected %zu", bytes, need);
+  HR_CUDA(cudaMemcpyAsync(dst, src, need, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost,
+                          s->stream));
+  HR_CUDA(cudaStreamSynchronize(s->stream));
+  return HR_OK;
+}
+
+hr_status hr_get_u(hr_solver* s, void* dst, size_t bytes, int32_t dst_on_device) {
+  return get_field(s, s ? s->a.Y[0] : nullptr, dst, bytes, dst_on_device);
+}
+
+hr_status hr_get_v(hr_solver* s, void* dst, size_t bytes, int32_t dst_on_device) {
+  return get_field(s, s ? s->a.Y[1] : nullptr, dst, bytes, dst_on_device);
+}
+
+hr_status hr_set_state(hr_solver* s, const void* u, const void* v, int32_t src_on_device) {
+  if (!s || !u || !v) return fail(HR_ERR_INVALID_ARG, "NULL argument");
+  const size_t need = (size_t)s->g.ntot * s->scalar_bytes;
+  const cudaMemcpyKind kind = src_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+  HR_CUDA(cudaMemcpyAsync(s->a.Y[0], u, need, kind, s->stream));
+  HR_CUDA(cudaMemcpyAsync(s->a.Y[1], v, need, kind, s->stream));
+  HR_CUDA(hrk_inner_fill(s, s->a.Y[0], s->a.Y[1]));
+  if (!src_on_device) HR_CUDA(cudaStreamSynchronize(s->stream));
+  return HR_OK;
+}
+
+hr_status hr_eval_rhs(hr_solver* s, void* ku_dev, void* kv_dev) {
+  if (!s || !ku_dev || !kv_dev) return fail(HR_ERR_INVALID_ARG, "NULL argument");
+  HR_CUDA(hrk_eval_rhs(s, ku_dev, kv_dev));
+  return HR_OK;
+}
+
+hr_status hr_get_source(hr_solver* s, void* psi_host, void* S_host) {
+  if (!s) return fail(HR_ERR_INVALID_ARG, "solver is NULL");
+  const size_t need = (size_t)s->g.ntot * s->scalar_bytes;
+  if (psi_host) HR_CUDA(cudaMemcpyAsync(psi_host, s->a.psi, need, cudaMemcpyDeviceToHost, s->stream));
+  if (S_host) HR_CUDA(cudaMemcpyAsync(S_host, s->a.S, need, cudaMemcpyDeviceToHost, s->stream));
+  HR_CUDA(cudaStreamSynchronize(s->stream));
+  return HR_OK;
+}
+
+hr_status hr_get_bc_lists(hr_solver* s, int32_t* inner_dst, int32_t* inner_src, int64_t* n_inner,
+                          int32_t* outer_idx, int64_t* n_outer) {
+  if (!s) return fail(HR_ERR_INVALID_ARG, "solver is NULL");
+  if (n_inner) *n_inner = (int64_t)s->inner_dst.size();
+  if (n_outer) *n_outer = (int64_t)s->outer_idx.size();
+  if (inner_dst) memcpy(inner_dst, s->inner_dst.data(), s->inner_dst.size() * 4);
+  if (inner_src) memcpy(inner_src, s->inner_src.data(), s->inner_src.size() * 4);
+  if (outer_idx) memcpy(outer_idx, s->outer_idx.data(), s->outer_idx.size() * 4);
+  return HR_OK;
+}
+
+hr_status hr_get_info(hr_solver* s, double* dt, double* dsmin, int32_t* nghosts, int32_t* T,
+                      int64_t* total_pts) {
+  if (!s) return fail(HR_ERR_INVALID_ARG, "solver is NULL");
+  if (dt) *dt = s->dt;
+  if (dsmin) *dsmin = s->dsmin;
+  if (nghosts) *nghosts = s->g.ng;
+  if (T) {
+    T[0] = s->g.T0;
+    T[1] = s->g.T1;
+    T[2] = s->g.T2;
+  }
+  if (total_pts) *total_pts = s->g.ntot;
+  return HR_OK;
+}
+
+hr_status hr_launches_per_step(hr_solver* s, int32_t* n) {
+  if (!s || !n) return fail(HR_ERR_INVALID_ARG, "NULL argument");
+  *n = s->launches_per_step;
+  return HR_OK;
+}
+
+}  // extern "C"

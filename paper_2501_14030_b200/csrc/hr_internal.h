@@ -1,0 +1,90 @@
+// hr_internal.h -- solver object and the launcher interface between hr_api.cu (host logic) and
+// hr_kernels.cu (device code).  Product code: shares nothing with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/hr.h"
+
+#define HR_MAX_NG 6
+
+// Device-side view of one solver: everything a kernel needs, passed by value (__grid_constant__).
+// Grid functions are stored with the public layout idx = i0 + T0 (i1 + T1 i2) (reading C8).
+struct HrGrid {
+  int32_t n0, n1, n2;  // interior points
+  int32_t ng;          // ghost layers = FD radius (C7)
+  int32_t T0, T1, T2;  // points per axis incl. ghosts
+  int64_t s1, s2;      // strides of i1 and i2 in scalars (T0, T0*T1)
+  int64_t ntot;
+  int64_t n_inner;
+  int32_t n_outer_cols;  // = ng: outer layers i0 in [n0+ng, T0)
+};
+
+// Pointers into the caller's workspace.  `void*` scalars are double or float per dtype.
+struct HrArrays {
+  void* Y[2];    // state (u, v)
+  void* A[2];    // stage buffer A
+  void* B[2];    // stage buffer B
+  void* ACC[2];  // running RK4 sum  Y + dt/6 k1 + dt/3 k2 + dt/3 k3
+  void* psi;     // psi_BL (C1)
+  void* S;       // (1/8) A~_ij A~^ij (C2)
+  // (i0,i1) planes, index i0 + T0 i1, working dtype (reading C4, C9, C12); FD weights are for
+  // unit spacing, so the 1/dx^a and 1/(dx^a)^2 factors are folded in here.
+  void* L00;  // g00 / dx0^2
+  void* L11;  // g11 / dx1^2
+  void* L22;  // g22 / dx2^2
+  void* L0;   // g0 / dx0
+  void* L1;   // g1 / dx1
+  void* C2;   // c^2
+  // outer radiation condition (C13), compact (ng x T1) arrays, index j + ng*i1, j = i0-(n0+ng):
+  void* RAD0;  // c * rad0 / (2 dx0)
+  void* RAD1;  // c * rad1 / (2 dx1)
+  void* RADI;  // c / r
+  double* Wvol;  // |h0 h1 h2| plane, always fp64 (C16)
+  int32_t* inner_dst;
+  int32_t* inner_src;
+  double* partials;  // residual partial sums: 2 doubles per block
+  double* result2;   // {sum w H^2, sum w}
+  // 1-D coordinate tables for the source kernel, fp64 (host libm values)
+  double *rho, *rhoz;          // T0: rho(x0); sqrt(rho^2 + b^2) (SymTP) or rho (spherical)
+  double *sinth, *costh;       // T1
+  double *sinph, *cosph;       // T2
+  double* punct;               // n_punctures x 10
+};
+
+struct hr_solver {
+  hr_params p;
+  std::vector<hr_puncture> punctures;
+  HrGrid g;
+  HrArrays a;
+  double dx[3];
+  double dt, dsmin;
+  int64_t n_outer;
+  std::vector<int32_t> inner_dst, inner_src, outer_idx;  // host copies (hr_get_bc_lists)
+  size_t scalar_bytes;
+  int max_partials;
+  cudaStream_t stream;
+  cudaGraphExec_t step_graph;  // one RK4 step = 4 x (fused kernel, inner fill)
+  int launches_per_step;
+  void* workspace;
+  size_t workspace_bytes;
+};
+
+// ---- hr_kernels.cu ----
+// All launchers return the cudaError_t of the launch (cudaGetLastError).
+cudaError_t hrk_source(const hr_solver* s);
+// stage = 1..4: fused [RHS at interior + radiation at outer] + RK combine, then inner fill of
+// the array written by that stage.
+cudaError_t hrk_substep(const hr_solver* s, int stage);
+// k = full Alg. 1 l.13-14 evaluation of the current state into ku, kv (N_tot each).
+cudaError_t hrk_eval_rhs(const hr_solver* s, void* ku, void* kv);
+// inner fill (C14) of f (N_tot scalars) / of the pair (fu, fv)
+cudaError_t hrk_inner_fill(const hr_solver* s, void* fu, void* fv);
+// residual partial sums + final deterministic pass into out2_dev
+cudaError_t hrk_residual(const hr_solver* s, int mode, double* out2_dev);
+int hrk_residual_blocks(const HrGrid& g);
+int hrk_launches_per_substep(const hr_solver* s);

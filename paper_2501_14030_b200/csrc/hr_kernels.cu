@@ -1,0 +1,444 @@
+// hr_kernels.cu -- device code of the hyperbolic-relaxation hot path for sm_100a.
+//
+//   a0  k_source        psi_BL and S = (1/8) A~_ij A~^ij, once        (C1, C2)
+//   a1  fused substep   RHS of Eq. 5 at interior points
+//   a2  fused substep   radiation condition at the outer points       (C13)
+//   a4  fused substep   RK4 combine (k never reaches HBM)              (C15)
+//   a3  k_inner_fill    inner (parity) ghosts through the index map   (C14)
+//   a5  k_residual      H and its grid L2 norm                        (C16)
+//
+// Product code: nothing here includes, links or calls oracle/.
+#include <cuda_runtime.h>
+
+#include "fd_tables.cuh"
+#include "hr_internal.h"
+
+namespace {
+
+// ------------------------------------------------------------------------------------------
+// arithmetic shared by the RHS and the residual
+// ------------------------------------------------------------------------------------------
+
+// (psi_BL + u)^-7 of Eq. 4/5: one reciprocal and four multiplies.
+template <typename T>
+__device__ __forceinline__ T pow_m7(T x) {
+  const T t = T(1) / x;
+  const T t2 = t * t;
+  const T t4 = t2 * t2;
+  return t4 * t2 * t;
+}
+
+template <typename T>
+struct StepArgs {
+  const T* in_u;  // stage input (stencil source)
+  const T* in_v;
+  const T* y_u;  // Y (needed by stages 2, 3; stage 1 has in == Y)
+  const T* y_v;
+  T* out_u;  // stages 1-3: next stage input; stage 4: Y; eval mode: k_u
+  T* out_v;
+  T* acc_u;
+  T* acc_v;
+  const T* psi;
+  const T* S;
+  const T *L00, *L11, *L22, *L0, *L1, *C2;
+  const T *RAD0, *RAD1, *RADI;
+  T eta;
+  T dt;
+};
+
+// Classic RK4 (C15) in running-sum form.  STAGE 0 = "store k" (hr_eval_rhs).
+//   1: out = Y + dt/2 k ; ACC  = Y + dt/6 k
+//   2: out = Y + dt/2 k ; ACC += dt/3 k
+//   3: out = Y + dt   k ; ACC += dt/3 k
+//   4: Y   = ACC + dt/6 k
+template <typename T, int STAGE>
+__device__ __forceinline__ void rk_combine(const StepArgs<T>& a, int64_t c, T ku, T kv, T in_u,
+                                           T in_v) {
+  if constexpr (STAGE == 0) {
+    a.out_u[c] = ku;
+    a.out_v[c] = kv;
+  } else if constexpr (STAGE == 1) {
+    const T h = a.dt * T(0.5), s = a.dt / T(6);
+    a.out_u[c] = in_u + h * ku;
+    a.out_v[c] = in_v + h * kv;
+    a.acc_u[c] = in_u + s * ku;
+    a.acc_v[c] = in_v + s * kv;
+  } else if constexpr (STAGE == 2 || STAGE == 3) {
+    const T h = (STAGE == 2) ? a.dt * T(0.5) : a.dt;
+    const T s = a.dt / T(3);
+    const T yu = a.y_u[c], yv = a.y_v[c];
+    const T au = a.acc_u[c], av = a.acc_v[c];
+    a.out_u[c] = yu + h * ku;
+    a.out_v[c] = yv + h * kv;
+    a.acc_u[c] = au + s * ku;
+    a.acc_v[c] = av + s * kv;
+  } else {
+    const T s = a.dt / T(6);
+    a.out_u[c] = a.acc_u[c] + s * ku;
+    a.out_v[c] = a.acc_v[c] + s * kv;
+  }
+}
+
+// Expanded curvilinear Laplacian (C4, C11, C12) with direct global loads of the stencil.
+template <typename T, int NG>
+__device__ __forceinline__ T laplacian_direct(const T* __restrict__ u, int64_t c, int64_t s1,
+                                              int64_t s2, T uc, T l00, T l11, T l22, T l0, T l1) {
+  using F = FdTable<NG>;
+  T d00 = T(F::d2(0)) * uc, d11 = d00, d22 = d00;
+  T d0 = T(0), d1 = T(0);
+#pragma unroll
+  for (int k = 1; k <= NG; ++k) {
+    const T a0 = u[c + k], b0 = u[c - k];
+    const T a1 = u[c + k * s1], b1 = u[c - k * s1];
+    const T a2 = u[c + k * s2], b2 = u[c - k * s2];
+    d00 += T(F::d2(k)) * (a0 + b0);
+    d11 += T(F::d2(k)) * (a1 + b1);
+    d22 += T(F::d2(k)) * (a2 + b2);
+    d0 += T(F::c1(k)) * (a0 - b0);
+    d1 += T(F::c1(k)) * (a1 - b1);
+  }
+  return l00 * d00 + l11 * d11 + l22 * d22 + l0 * d0 + l1 * d1;
+}
+
+// Radiation condition (C13) at an outer point c = (i0,i1,i2), j = i0 - (n0+ng):
+//   k_f = -c [ rad0 (3 f_i - 4 f_{i-1} + f_{i-2})/(2 dx0) + rad1 (f_{i1+1} - f_{i1-1})/(2 dx1) + f/r ]
+template <typename T>
+__device__ __forceinline__ T radiation_k(const T* __restrict__ f, int64_t c, int64_t s1, T r0,
+                                         T r1, T ri) {
+  const T fc = f[c];
+  const T d0 = T(3) * fc - T(4) * f[c - 1] + f[c - 2];
+  const T d1 = f[c + s1] - f[c - s1];
+  return -(r0 * d0 + r1 * d1 + ri * fc);
+}
+
+// ------------------------------------------------------------------------------------------
+// a1 + a2 + a4, direct-load arrangement: one thread per point, i0 along threadIdx.x
+// ------------------------------------------------------------------------------------------
+constexpr int DBX = 64, DBY = 4;
+
+template <typename T, int NG, int STAGE>
+__global__ void __launch_bounds__(DBX* DBY)
+    k_substep_direct(const __grid_constant__ HrGrid g, const __grid_constant__ StepArgs<T> a) {
+  const int i0 = NG + blockIdx.x * DBX + threadIdx.x;
+  const int i1 = NG + blockIdx.y * DBY + threadIdx.y;
+  const int i2 = NG + blockIdx.z;
+  if (i0 >= g.T0 || i1 >= g.n1 + NG) return;
+  const int64_t c = i0 + g.s1 * i1 + g.s2 * i2;
+  const T uc = a.in_u[c], vc = a.in_v[c];
+  T ku, kv;
+  if (i0 < g.n0 + NG) {
+    const int64_t q = i0 + (int64_t)g.T0 * i1;
+    const T lap = laplacian_direct<T, NG>(a.in_u, c, g.s1, g.s2, uc, a.L00[q], a.L11[q], a.L22[q],
+                                          a.L0[q], a.L1[q]);
+    ku = vc - a.eta * uc;
+    kv = a.C2[q] * (lap + a.S[c] * pow_m7(a.psi[c] + uc));
+  } else {
+    const int qo = (i0 - (g.n0 + NG)) + NG * i1;
+    const T r0 = a.RAD0[qo], r1 = a.RAD1[qo], ri = a.RADI[qo];
+    ku = radiation_k(a.in_u, c, g.s1, r0, r1, ri);
+    kv = radiation_k(a.in_v, c, g.s1, r0, r1, ri);
+  }
+  rk_combine<T, STAGE>(a, c, ku, kv, uc, vc);
+}
+
+// ------------------------------------------------------------------------------------------
+// a3: inner ghosts through the precomputed index map (C14), parity +1
+// ------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(256)
+    k_inner_fill(T* __restrict__ fu, T* __restrict__ fv, const int32_t* __restrict__ dst,
+                 const int32_t* __restrict__ src, int64_t n) {
+  const int64_t m = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (m >= n) return;
+  const int32_t d = dst[m], s = src[m];
+  fu[d] = fu[s];
+  if (fv) fv[d] = fv[s];
+}
+
+// ------------------------------------------------------------------------------------------
+// a5: H at interior points, weighted squares reduced warp -> block -> one partial per block
+// ------------------------------------------------------------------------------------------
+constexpr int RBX = 64, RBY = 4;
+
+template <typename T, int NG>
+__global__ void __launch_bounds__(RBX* RBY)
+    k_residual(const __grid_constant__ HrGrid g, const T* __restrict__ u,
+               const T* __restrict__ psi, const T* __restrict__ S, const T* __restrict__ L00,
+               const T* __restrict__ L11, const T* __restrict__ L22, const T* __restrict__ L0,
+               const T* __restrict__ L1, const double* __restrict__ W, int mode,
+               double* __restrict__ partials) {
+  const int i0 = NG + blockIdx.x * RBX + threadIdx.x;
+  const int i1 = NG + blockIdx.y * RBY + threadIdx.y;
+  const int i2 = NG + blockIdx.z;
+  double num = 0.0, den = 0.0;
+  if (i0 < g.n0 + NG && i1 < g.n1 + NG) {
+    const int64_t c = i0 + g.s1 * i1 + g.s2 * i2;
+    const int64_t q = i0 + (int64_t)g.T0 * i1;
+    const T uc = u[c];
+    const T lap =
+        laplacian_direct<T, NG>(u, c, g.s1, g.s2, uc, L00[q], L11[q], L22[q], L0[q], L1[q]);
+    const T H = lap + S[c] * pow_m7(psi[c] + uc);
+    const double w = (mode == 0) ? W[q] : 1.0;
+    num = w * (double)H * (double)H;
+    den = w;
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    num += __shfl_down_sync(0xffffffffu, num, o);
+    den += __shfl_down_sync(0xffffffffu, den, o);
+  }
+  __shared__ double sh[2][RBX * RBY / 32];
+  const int tid = threadIdx.y * RBX + threadIdx.x;
+  if ((tid & 31) == 0) {
+    sh[0][tid >> 5] = num;
+    sh[1][tid >> 5] = den;
+  }
+  __syncthreads();
+  if (tid == 0) {
+    double a = 0.0, b = 0.0;
+#pragma unroll
+    for (int w = 0; w < RBX * RBY / 32; ++w) {
+      a += sh[0][w];
+      b += sh[1][w];
+    }
+    const int64_t bid = blockIdx.x + (int64_t)gridDim.x * (blockIdx.y + (int64_t)gridDim.y * blockIdx.z);
+    partials[2 * bid] = a;
+    partials[2 * bid + 1] = b;
+  }
+}
+
+// Final pass: one block, fixed order (thread t sums partials t, t+1024, ...; then a tree).
+__global__ void __launch_bounds__(1024)
+    k_residual_final(const double* __restrict__ partials, int64_t nblocks, double* __restrict__ out2) {
+  __shared__ double sh[2][1024];
+  double a = 0.0, b = 0.0;
+  for (int64_t i = threadIdx.x; i < nblocks; i += 1024) {
+    a += partials[2 * i];
+    b += partials[2 * i + 1];
+  }
+  sh[0][threadIdx.x] = a;
+  sh[1][threadIdx.x] = b;
+  __syncthreads();
+  for (int o = 512; o > 0; o >>= 1) {
+    if ((int)threadIdx.x < o) {
+      sh[0][threadIdx.x] += sh[0][threadIdx.x + o];
+      sh[1][threadIdx.x] += sh[1][threadIdx.x + o];
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    out2[0] = sh[0][0];
+    out2[1] = sh[1][0];
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// a0: constant source terms, fp64 arithmetic, stored in the working precision (C1, C2, C19)
+// ------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(256)
+    k_source(const __grid_constant__ HrGrid g, const double* __restrict__ rho,
+             const double* __restrict__ rhoz, const double* __restrict__ sinth,
+             const double* __restrict__ costh, const double* __restrict__ sinph,
+             const double* __restrict__ cosph, const double* __restrict__ punct, int npunct,
+             double ox, double oy, double oz, T* __restrict__ psi_out, T* __restrict__ S_out,
+             int* __restrict__ bad_flag) {
+  const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= g.ntot) return;
+  const int i0 = (int)(c % g.T0);
+  const int i1 = (int)((c / g.T0) % g.T1);
+  const int i2 = (int)(c / g.s2);
+  // grid point in Cartesian coordinates (C4) + grid centre (C6)
+  const double rs = rho[i0] * sinth[i1];
+  const double x = rs * cosph[i2] + ox;
+  const double y = rs * sinph[i2] + oy;
+  const double z = rhoz[i0] * costh[i1] + oz;
+  double psi = 1.0;
+  double axx = 0, ayy = 0, azz = 0, axy = 0, axz = 0, ayz = 0;
+  for (int p = 0; p < npunct; ++p) {
+    const double* pp = punct + 10 * p;
+    const double m = pp[0];
+    const double dx = x - pp[1], dy = y - pp[2], dz = z - pp[3];
+    const double Px = pp[4], Py = pp[5], Pz = pp[6];
+    const double Sx = pp[7], Sy = pp[8], Sz = pp[9];
+    const double r2 = dx * dx + dy * dy + dz * dz;
+    const double r = sqrt(r2);
+    const double ir = 1.0 / r;
+    psi += 0.5 * m * ir;  // Brandt-Bruegmann psi_BL = 1 + sum m/(2r)
+    const double nx = dx * ir, ny = dy * ir, nz = dz * ir;
+    const double Pn = Px * nx + Py * ny + Pz * nz;
+    // (S x n)
+    const double cx = Sy * nz - Sz * ny, cy = Sz * nx - Sx * nz, cz = Sx * ny - Sy * nx;
+    const double fP = 1.5 * ir * ir;       // 3 / (2 r^2)
+    const double fS = 3.0 * ir * ir * ir;  // 3 / r^3
+    // Bowen-York: fP [P^i n^j + P^j n^i - (delta^ij - n^i n^j) P.n] + fS [(Sxn)^i n^j + (Sxn)^j n^i]
+    axx += fP * (2.0 * Px * nx - (1.0 - nx * nx) * Pn) + fS * (2.0 * cx * nx);
+    ayy += fP * (2.0 * Py * ny - (1.0 - ny * ny) * Pn) + fS * (2.0 * cy * ny);
+    azz += fP * (2.0 * Pz * nz - (1.0 - nz * nz) * Pn) + fS * (2.0 * cz * nz);
+    axy += fP * (Px * ny + Py * nx + nx * ny * Pn) + fS * (cx * ny + cy * nx);
+    axz += fP * (Px * nz + Pz * nx + nx * nz * Pn) + fS * (cx * nz + cz * nx);
+    ayz += fP * (Py * nz + Pz * ny + ny * nz * Pn) + fS * (cy * nz + cz * ny);
+  }
+  const double AA = axx * axx + ayy * ayy + azz * azz + 2.0 * (axy * axy + axz * axz + ayz * ayz);
+  const double Sval = 0.125 * AA;
+  if (!isfinite(psi) || !isfinite(Sval)) atomicOr(bad_flag, 1);
+  psi_out[c] = (T)psi;
+  S_out[c] = (T)Sval;
+}
+
+// ------------------------------------------------------------------------------------------
+// host-side dispatch
+// ------------------------------------------------------------------------------------------
+template <typename T>
+StepArgs<T> make_args(const hr_solver* s, int stage, void* ku, void* kv) {
+  const HrArrays& a = s->a;
+  StepArgs<T> r{};
+  auto P = [](void* p) { return static_cast<T*>(p); };
+  switch (stage) {
+    case 0:  // eval: in = Y, out = k
+      r.in_u = P(a.Y[0]); r.in_v = P(a.Y[1]); r.out_u = P(ku); r.out_v = P(kv);
+      break;
+    case 1:
+      r.in_u = P(a.Y[0]); r.in_v = P(a.Y[1]); r.out_u = P(a.A[0]); r.out_v = P(a.A[1]);
+      break;
+    case 2:
+      r.in_u = P(a.A[0]); r.in_v = P(a.A[1]); r.out_u = P(a.B[0]); r.out_v = P(a.B[1]);
+      break;
+    case 3:
+      r.in_u = P(a.B[0]); r.in_v = P(a.B[1]); r.out_u = P(a.A[0]); r.out_v = P(a.A[1]);
+      break;
+    default:
+      r.in_u = P(a.A[0]); r.in_v = P(a.A[1]); r.out_u = P(a.Y[0]); r.out_v = P(a.Y[1]);
+      break;
+  }
+  r.y_u = P(a.Y[0]); r.y_v = P(a.Y[1]);
+  r.acc_u = P(a.ACC[0]); r.acc_v = P(a.ACC[1]);
+  r.psi = P(a.psi); r.S = P(a.S);
+  r.L00 = P(a.L00); r.L11 = P(a.L11); r.L22 = P(a.L22); r.L0 = P(a.L0); r.L1 = P(a.L1);
+  r.C2 = P(a.C2); r.RAD0 = P(a.RAD0); r.RAD1 = P(a.RAD1); r.RADI = P(a.RADI);
+  r.eta = (T)s->p.eta;
+  r.dt = (T)s->dt;
+  return r;
+}
+
+template <typename T, int NG>
+cudaError_t launch_substep_direct(const hr_solver* s, int stage, void* ku, void* kv) {
+  const HrGrid& g = s->g;
+  const StepArgs<T> a = make_args<T>(s, stage, ku, kv);
+  const dim3 block(DBX, DBY, 1);
+  const dim3 grid((g.n0 + NG + DBX - 1) / DBX, (g.n1 + DBY - 1) / DBY, g.n2);
+  switch (stage) {
+    case 0: k_substep_direct<T, NG, 0><<<grid, block, 0, s->stream>>>(g, a); break;
+    case 1: k_substep_direct<T, NG, 1><<<grid, block, 0, s->stream>>>(g, a); break;
+    case 2: k_substep_direct<T, NG, 2><<<grid, block, 0, s->stream>>>(g, a); break;
+    case 3: k_substep_direct<T, NG, 3><<<grid, block, 0, s->stream>>>(g, a); break;
+    default: k_substep_direct<T, NG, 4><<<grid, block, 0, s->stream>>>(g, a); break;
+  }
+  return cudaGetLastError();
+}
+
+template <typename T>
+cudaError_t dispatch_substep(const hr_solver* s, int stage, void* ku, void* kv) {
+  switch (s->g.ng) {
+    case 1: return launch_substep_direct<T, 1>(s, stage, ku, kv);
+    case 2: return launch_substep_direct<T, 2>(s, stage, ku, kv);
+    case 3: return launch_substep_direct<T, 3>(s, stage, ku, kv);
+    case 4: return launch_substep_direct<T, 4>(s, stage, ku, kv);
+    case 5: return launch_substep_direct<T, 5>(s, stage, ku, kv);
+    case 6: return launch_substep_direct<T, 6>(s, stage, ku, kv);
+  }
+  return cudaErrorInvalidValue;
+}
+
+template <typename T>
+cudaError_t inner_fill_t(const hr_solver* s, void* fu, void* fv) {
+  const int64_t n = s->g.n_inner;
+  if (n == 0) return cudaSuccess;
+  const int blocks = (int)((n + 255) / 256);
+  k_inner_fill<T><<<blocks, 256, 0, s->stream>>>(static_cast<T*>(fu), static_cast<T*>(fv),
+                                                  s->a.inner_dst, s->a.inner_src, n);
+  return cudaGetLastError();
+}
+
+template <typename T, int NG>
+cudaError_t launch_residual(const hr_solver* s, int mode, double* out2) {
+  const HrGrid& g = s->g;
+  const HrArrays& a = s->a;
+  auto P = [](void* p) { return static_cast<const T*>(p); };
+  const dim3 block(RBX, RBY, 1);
+  const dim3 grid((g.n0 + RBX - 1) / RBX, (g.n1 + RBY - 1) / RBY, g.n2);
+  k_residual<T, NG><<<grid, block, 0, s->stream>>>(g, P(a.Y[0]), P(a.psi), P(a.S), P(a.L00),
+                                                    P(a.L11), P(a.L22), P(a.L0), P(a.L1), a.Wvol,
+                                                    mode, a.partials);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  const int64_t nb = (int64_t)grid.x * grid.y * grid.z;
+  k_residual_final<<<1, 1024, 0, s->stream>>>(a.partials, nb, out2);
+  return cudaGetLastError();
+}
+
+template <typename T>
+cudaError_t dispatch_residual(const hr_solver* s, int mode, double* out2) {
+  switch (s->g.ng) {
+    case 1: return launch_residual<T, 1>(s, mode, out2);
+    case 2: return launch_residual<T, 2>(s, mode, out2);
+    case 3: return launch_residual<T, 3>(s, mode, out2);
+    case 4: return launch_residual<T, 4>(s, mode, out2);
+    case 5: return launch_residual<T, 5>(s, mode, out2);
+    case 6: return launch_residual<T, 6>(s, mode, out2);
+  }
+  return cudaErrorInvalidValue;
+}
+
+}  // namespace
+
+int hrk_residual_blocks(const HrGrid& g) {
+  return ((g.n0 + RBX - 1) / RBX) * ((g.n1 + RBY - 1) / RBY) * g.n2;
+}
+
+int hrk_launches_per_substep(const hr_solver* s) { return s->g.n_inner > 0 ? 2 : 1; }
+
+cudaError_t hrk_inner_fill(const hr_solver* s, void* fu, void* fv) {
+  return s->p.dtype == HR_F64 ? inner_fill_t<double>(s, fu, fv) : inner_fill_t<float>(s, fu, fv);
+}
+
+cudaError_t hrk_substep(const hr_solver* s, int stage) {
+  cudaError_t e = s->p.dtype == HR_F64 ? dispatch_substep<double>(s, stage, nullptr, nullptr)
+                                       : dispatch_substep<float>(s, stage, nullptr, nullptr);
+  if (e != cudaSuccess) return e;
+  // a3 on the array this stage wrote (bitwise equivalent to filling k, C15)
+  void* const* out = (stage == 1 || stage == 3) ? s->a.A : (stage == 2 ? s->a.B : s->a.Y);
+  return hrk_inner_fill(s, out[0], out[1]);
+}
+
+cudaError_t hrk_eval_rhs(const hr_solver* s, void* ku, void* kv) {
+  cudaError_t e = s->p.dtype == HR_F64 ? dispatch_substep<double>(s, 0, ku, kv)
+                                       : dispatch_substep<float>(s, 0, ku, kv);
+  if (e != cudaSuccess) return e;
+  return hrk_inner_fill(s, ku, kv);
+}
+
+cudaError_t hrk_residual(const hr_solver* s, int mode, double* out2_dev) {
+  return s->p.dtype == HR_F64 ? dispatch_residual<double>(s, mode, out2_dev)
+                              : dispatch_residual<float>(s, mode, out2_dev);
+}
+
+cudaError_t hrk_source(const hr_solver* s) {
+  const HrGrid& g = s->g;
+  const HrArrays& a = s->a;
+  const int blocks = (int)((g.ntot + 255) / 256);
+  int* flag = reinterpret_cast<int*>(a.result2);  // reused as the bad-point flag during create
+  cudaError_t e = cudaMemsetAsync(flag, 0, sizeof(int), s->stream);
+  if (e != cudaSuccess) return e;
+  if (s->p.dtype == HR_F64)
+    k_source<double><<<blocks, 256, 0, s->stream>>>(
+        g, a.rho, a.rhoz, a.sinth, a.costh, a.sinph, a.cosph, a.punct, s->p.n_punctures,
+        s->p.origin[0], s->p.origin[1], s->p.origin[2], static_cast<double*>(a.psi),
+        static_cast<double*>(a.S), flag);
+  else
+    k_source<float><<<blocks, 256, 0, s->stream>>>(
+        g, a.rho, a.rhoz, a.sinth, a.costh, a.sinph, a.cosph, a.punct, s->p.n_punctures,
+        s->p.origin[0], s->p.origin[1], s->p.origin[2], static_cast<float*>(a.psi),
+        static_cast<float*>(a.S), flag);
+  return cudaGetLastError();
+}
