@@ -1,0 +1,406 @@
+"""bench.py -- throughput of the hyperbolic-relaxation hot path on B200 (one JSON line on stdout).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload config3] [--impl reference]
+
+A "step" is one pass of the whole hot path (Alg. 1 l.9-16) over
+the workload: the residual H + its L2 norm (a5) followed by one RK4 step = 4 x [fused RHS +
+radiation condition + RK combine (a1, a2, a4), inner ghost fill (a3)].  The one-time pieces (a0
+source kernel, a6 step constants) run in hr_create, outside the timed region.
+
+  metric  grid-point RK4 substep updates/s = N_int * 4 * K / (device time of K steps)
+  value   fp64, state resident in HBM, timed with CUDA events on the solver's stream
+  f32     the same workload in fp32 (BASELINE.json asks for both precisions)
+  e2e     the same steps through the C ABI with HOST buffers: every step copies (u, v) from pinned
+          host memory (hr_set_state, host pointers), runs the step and reads the residual back
+  roofline  dominant kernel (the fused substep): algorithmic bytes 10 w per interior point-substep
+           / mean launch duration measured here by hr_profile_step
+  cpu_baseline  the CPU oracle (oracle/, test infrastructure) timed on this box's host cores
+
+N > 1 (torchrun): the path does not shard ("replicas only"): every rank
+advances an independent replica of the workload, no data-path collective; value = all ranks' units
+/ max-over-ranks time.
+
+`--impl reference` times the CPU oracle as it stands on the same workload, metric and unit (rank 0
+only).  There is no installable reference for this paper.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+import hr_workloads as W  # noqa: E402
+
+METRIC = "grid-point RK4 substep updates/s"
+UNIT = "point-substeps/s"
+
+
+def workload(name: str) -> dict:
+    if name.startswith("config"):
+        return W.config(int(name[6:]))
+    if name.startswith("sweep"):  # sweep<idx>:<N0>x<N1>x<N2>:<coord>:<order>
+        idx, n, coord, order = name[5:].split(":")
+        return W.sweep_point(int(idx), tuple(int(x) for x in n.split("x")), coord, int(order))
+    raise SystemExit(f"unknown workload {name}")
+
+
+def config_dict(p: dict, name: str, n_gpus: int) -> dict:
+    ng = p["fd_order"] // 2
+    T = [x + 2 * ng for x in p["n"]]
+    ntot = T[0] * T[1] * T[2]
+    return {"workload": f"BASELINE.json {name.replace('config', 'configs[') + ']' if name.startswith('config') else name}",
+            "coord": p["coord"], "n_interior": list(p["n"]), "fd_order": p["fd_order"],
+            "n_tot_points": ntot, "eta": p["eta"], "cfl": p["cfl"],
+            "step": "residual (H + L2 norm) + 1 RK4 step = 4 x (fused RHS+radiation+RK combine, inner fill)",
+            "l2": "inputs larger than L2 (10 grid functions = %.0f MB fp64)" % (10 * ntot * 8 / 1e6)
+            if 10 * ntot * 4 > 126e6 else "working set fits L2 (%.1f MB fp64): L2 flushed between timed steps"
+            % (10 * ntot * 8 / 1e6),
+            "parallelism": "replicas only x%d" % n_gpus}
+
+
+# ------------------------------------------------------------------------------------------------
+# clocks during the timed region (profiling recipe's nvidia-smi line)
+# ------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.rows = []
+        self.proc = None
+        self.thread = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                 "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._read, daemon=True)
+        self.thread.start()
+
+    def _read(self):
+        for line in self.proc.stdout:
+            f = [x.strip() for x in line.split(",")]
+            if len(f) >= 9:
+                self.rows.append(f)
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for f in self.rows:
+            try:
+                sm.append(float(f[1]))
+                mx.append(float(f[2]))
+                power.append(float(f[3]))
+            except ValueError:
+                continue
+            for nme, val in zip(names, f[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(nme)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm),
+                "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------------
+# the CPU oracle legs (cpu_baseline and --impl reference): the only places that touch oracle/
+# ------------------------------------------------------------------------------------------------
+def oracle_step_seconds(p: dict, n_rk4: int, reps: int):
+    """Seconds per [residual + n_rk4 RK4 steps] of the fp64 oracle on workload p, `reps` times."""
+    from oracle import hr_oracle
+    o = hr_oracle.Oracle(p)
+    u = np.zeros(o.ntot)
+    v = np.zeros(o.ntot)
+    times = []
+    for _ in range(reps):
+        t0 = time.perf_counter()
+        o.residual(u, 0)
+        u, v = o.step(u, v, n_rk4)
+        times.append(time.perf_counter() - t0)
+    return times, o, hr_oracle.num_threads()
+
+
+def cpu_baseline(p: dict, name: str) -> dict:
+    t0 = time.perf_counter()
+    times, o, threads = oracle_step_seconds(p, 1, 1)  # calibrate (also warms the pages)
+    n = max(1, min(50, int(12.0 / max(times[0], 1e-3))))
+    times, o, threads = oracle_step_seconds(p, 1, n)
+    per = float(np.mean(times))
+    return {"value": o.n_int * 4 / per, "unit": UNIT, "cores": threads, "kind": "oracle",
+            "sample": f"{n} x (residual + 1 RK4 step) of {name} in fp64 on the full grid, "
+                      f"{per:.3f} s each, u = v = 0 start; total incl. oracle set-up "
+                      f"{time.perf_counter() - t0:.1f} s"}
+
+
+def run_reference(args, p, name):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import hr_oracle
+    o = hr_oracle.Oracle(p)
+    threads = hr_oracle.num_threads()
+    u = np.zeros(o.ntot)
+    v = np.zeros(o.ntot)
+
+    def one():
+        nonlocal u, v
+        o.residual(u, 0)
+        u, v = o.step(u, v, 1)
+
+    for _ in range(args.warmup):
+        one()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        one()
+    dt = time.perf_counter() - t0
+    value = o.n_int * 4 * args.steps / dt
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": config_dict(p, name, args.gpus),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle",
+                             "sample": f"{args.steps} x (residual + 1 RK4 step) of {name}, full grid, fp64"},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------
+# the CUDA path
+# ------------------------------------------------------------------------------------------------
+def time_resident(torch, hr, p, dtype, steps, warmup, dist, flush_l2):
+    """K timed steps with the state resident in HBM; returns (seconds max over ranks, solver)."""
+    s = hr.Solver(p, dtype=dtype, residual_mode=0)
+    out2 = torch.zeros(2, dtype=torch.float64, device=s.device)
+    flush = None
+    if flush_l2:
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device=s.device)
+
+    def one():
+        s.hr_residual_async(0, out2)
+        s.hr_step(1)
+
+    for _ in range(warmup):
+        one()
+    s.synchronize()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    if flush is None:
+        e0 = torch.cuda.Event(enable_timing=True)
+        e1 = torch.cuda.Event(enable_timing=True)
+        e0.record(s.stream)
+        for _ in range(steps):
+            one()
+        e1.record(s.stream)
+        e1.synchronize()
+        ms = e0.elapsed_time(e1)
+    else:  # L2-resident workload: flush between timed steps, time each step by its own event pair
+        ms = 0.0
+        evs = []
+        for _ in range(steps):
+            with torch.cuda.stream(s.stream):
+                flush.zero_()
+            e0 = torch.cuda.Event(enable_timing=True)
+            e1 = torch.cuda.Event(enable_timing=True)
+            e0.record(s.stream)
+            one()
+            e1.record(s.stream)
+            evs.append((e0, e1))
+        s.synchronize()
+        ms = sum(a.elapsed_time(b) for a, b in evs)
+    torch.cuda.synchronize()
+    sec = ms * 1e-3
+    if dist is not None:
+        t = torch.tensor([sec], dtype=torch.float64, device=s.device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.barrier()
+        sec = float(t.item())
+    return sec, s
+
+
+def time_e2e(torch, s, steps, warmup, dist):
+    """Same step through the C ABI with host buffers: H2D of (u, v) from pinned memory, the step,
+    D2H of the residual.  Returns (seconds max over ranks, h2d bytes, d2h bytes)."""
+    u = torch.zeros(s.ntot, dtype=s.tdtype).pin_memory()
+    v = torch.zeros(s.ntot, dtype=s.tdtype).pin_memory()
+
+    def one():
+        s.hr_set_state_pinned(u, v)     # hr_set_state with host pointers: H2D + ghost fill
+        s.hr_step(1)
+        return s.hr_residual(0)         # D2H of {sum w H^2, sum w}, synchronises
+
+    for _ in range(warmup):
+        one()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    t0 = time.perf_counter()
+    e0 = torch.cuda.Event(enable_timing=True)
+    e1 = torch.cuda.Event(enable_timing=True)
+    e0.record(s.stream)
+    for _ in range(steps):
+        one()
+    e1.record(s.stream)
+    e1.synchronize()
+    sec = max(e0.elapsed_time(e1) * 1e-3, 0.0)
+    wall = time.perf_counter() - t0
+    sec = max(sec, wall) if wall > 0 else sec  # host-side marshalling counts too
+    if dist is not None:
+        t = torch.tensor([sec], dtype=torch.float64, device=s.device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        sec = float(t.item())
+    w = 8 if s.dtype == "f64" else 4
+    return sec, 2 * s.ntot * w, 16
+
+
+def roofline(s, prof_ms, peak, peak_src):
+    """Fused substep kernel: 10 w algorithmic bytes per interior point-substep (8w, 12w, 12w, 8w for
+    stages 1..4) x N_int points per launch / mean launch duration."""
+    w = 8 if s.dtype == "f64" else 4
+    mean_ms = sum(prof_ms[:4]) / 4.0
+    bytes_per_launch = 10 * w * s.n_int
+    achieved = bytes_per_launch / (mean_ms * 1e-3) / 1e9
+    return {"bound": "hbm", "kernel": "fused substep (RHS + radiation + RK combine), mean of the 4 stages",
+            "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+            "peak_source": peak_src, "algorithmic_bytes_per_launch": bytes_per_launch,
+            "launch_ms": {"stage1": prof_ms[0], "stage2": prof_ms[1], "stage3": prof_ms[2],
+                          "stage4": prof_ms[3], "inner_fill_x4": prof_ms[4], "residual": prof_ms[5]},
+            "substep_kernel_share_of_step": sum(prof_ms[:4]) / sum(prof_ms),
+            "traffic": None}
+
+
+def load_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except (OSError, KeyError, ValueError):
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def load_traffic(dtype):
+    """dram bytes per launch of the fused kernel from the committed ncu --set full capture, if any."""
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        with open(path) as f:
+            return json.load(f).get(dtype)
+    except (OSError, ValueError):
+        return None
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--workload", default="config3")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-f32", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    name = args.workload
+    p = workload(name)
+
+    if args.impl == "reference":
+        run_reference(args, p, name)
+        return
+
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the hot path has no CPU fallback")
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    import paper_2501_14030_b200 as hr
+
+    T = [x + p["fd_order"] for x in p["n"]]
+    ntot = T[0] * T[1] * T[2]
+    n_int = p["n"][0] * p["n"][1] * p["n"][2]
+    flush_l2 = 10 * ntot * 8 <= 126e6  # fp64 working set fits L2 -> flush between timed steps
+    peak, peak_src = load_peak()
+
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    sec64, s64 = time_resident(torch, hr, p, "f64", args.steps, args.warmup, dist, flush_l2)
+    launches_per_step = s64.launches_per_step + 2  # + residual kernel and its final pass
+    clocks = sampler.stop() if rank == 0 else None
+    value = world * n_int * 4 * args.steps / sec64
+
+    prof64 = s64.hr_profile_step(min(args.steps, 20), True)
+    roof = roofline(s64, prof64, peak, peak_src)
+    roof["traffic"] = load_traffic("f64")
+    sec_e2e, h2d, d2h = time_e2e(torch, s64, max(3, min(args.steps, 10)), 3, dist)
+    e2e_steps = max(3, min(args.steps, 10))
+    e2e = {"value": world * n_int * 4 * e2e_steps / sec_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d,
+           "d2h_bytes_per_step": d2h, "steps": e2e_steps,
+           "what": "per step: hr_set_state(u, v from pinned host memory) + residual + 1 RK4 step + "
+                   "residual read back to the host"}
+    s64.close()
+    del s64
+    torch.cuda.empty_cache()
+
+    f32 = None
+    if not args.no_f32:
+        sec32, s32 = time_resident(torch, hr, p, "f32", args.steps, args.warmup, dist,
+                                   10 * ntot * 4 <= 126e6)
+        prof32 = s32.hr_profile_step(min(args.steps, 20), True)
+        r32 = roofline(s32, prof32, peak, peak_src)
+        r32["traffic"] = load_traffic("f32")
+        f32 = {"value": world * n_int * 4 * args.steps / sec32, "unit": UNIT,
+               "ms_per_step": 1e3 * sec32 / args.steps, "roofline": r32}
+        s32.close()
+        del s32
+
+    if dist is not None:
+        dist.barrier()
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * sec64 / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": config_dict(p, name, world), "clocks": clocks, "e2e": e2e,
+            "gpu_launches": launches_per_step * args.steps, "roofline": roof, "f32": f32,
+            "library": hr.hr_version()}
+    if world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(p, name)
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -158,6 +158,14 @@ HR_API hr_status hr_host_setup(const hr_params* p, double* dt, double* dsmin, in
                                int64_t* n_outer, int32_t* inner_dst, int32_t* inner_src,
                                int32_t* outer_idx, double* planes7, double* outer3);
 
+/* Measurement hook (bench.py's roofline object): advances n_steps RK4 steps (1..4096) with plain
+ * launches of the same kernels hr_step uses, each bracketed by a CUDA event pair on the solver's
+ * stream, preceded per step by one residual evaluation (Alg. 1 l.9-11) if with_residual != 0.
+ * ms6 (host pointer, 6 doubles) receives the mean milliseconds per RK4 step spent in
+ * { fused substep kernel of stage 1, 2, 3, 4, the four inner fills together, residual }.
+ * Synchronises the stream. */
+HR_API hr_status hr_profile_step(hr_solver* s, int64_t n_steps, int32_t with_residual, double* ms6);
+
 /* Number of kernel launches one hr_step(1) enqueues (for bench.py's gpu_launches). */
 HR_API hr_status hr_launches_per_step(hr_solver* s, int32_t* n);
 

@@ -635,6 +635,53 @@ hr_status hr_get_info(hr_solver* s, double* dt, double* dsmin, int32_t* nghosts,
   return HR_OK;
 }
 
+hr_status hr_profile_step(hr_solver* s, int64_t n_steps, int32_t with_residual, double* ms6) {
+  if (!s || !ms6) return fail(HR_ERR_INVALID_ARG, "NULL argument");
+  if (n_steps < 1 || n_steps > 4096) return fail(HR_ERR_INVALID_ARG, "n_steps must be in 1..4096");
+  // one event pair per launch; elapsed times are read after a single synchronisation at the end
+  const int per_step = 8 + (with_residual ? 1 : 0);
+  std::vector<cudaEvent_t> ev((size_t)n_steps * per_step * 2, nullptr);
+  struct Cleanup {
+    std::vector<cudaEvent_t>& ev;
+    ~Cleanup() { for (cudaEvent_t e : ev) if (e) cudaEventDestroy(e); }
+  } cleanup{ev};
+  for (auto& e : ev) HR_CUDA(cudaEventCreate(&e));
+  size_t k = 0;
+  for (int64_t it = 0; it < n_steps; ++it) {
+    if (with_residual) {
+      HR_CUDA(cudaEventRecord(ev[k++], s->stream));
+      HR_CUDA(hrk_residual(s, s->p.residual_mode, s->a.result2));
+      HR_CUDA(cudaEventRecord(ev[k++], s->stream));
+    }
+    for (int stage = 1; stage <= 4; ++stage) {
+      HR_CUDA(cudaEventRecord(ev[k++], s->stream));
+      HR_CUDA(hrk_substep_main(s, stage));
+      HR_CUDA(cudaEventRecord(ev[k++], s->stream));
+      HR_CUDA(cudaEventRecord(ev[k++], s->stream));
+      HR_CUDA(hrk_substep_fill(s, stage));
+      HR_CUDA(cudaEventRecord(ev[k++], s->stream));
+    }
+  }
+  HR_CUDA(cudaStreamSynchronize(s->stream));
+  double acc[6] = {0, 0, 0, 0, 0, 0};
+  k = 0;
+  auto el = [&](size_t i, double& dst) -> cudaError_t {
+    float ms = 0.f;
+    cudaError_t e = cudaEventElapsedTime(&ms, ev[i], ev[i + 1]);
+    dst += ms;
+    return e;
+  };
+  for (int64_t it = 0; it < n_steps; ++it) {
+    if (with_residual) { HR_CUDA(el(k, acc[5])); k += 2; }
+    for (int stage = 1; stage <= 4; ++stage) {
+      HR_CUDA(el(k, acc[stage - 1])); k += 2;
+      HR_CUDA(el(k, acc[4])); k += 2;
+    }
+  }
+  for (int i = 0; i < 6; ++i) ms6[i] = acc[i] / (double)n_steps;
+  return HR_OK;
+}
+
 hr_status hr_launches_per_step(hr_solver* s, int32_t* n) {
   if (!s || !n) return fail(HR_ERR_INVALID_ARG, "NULL argument");
   *n = s->launches_per_step;

@@ -80,6 +80,9 @@ cudaError_t hrk_source(const hr_solver* s);
 // stage = 1..4: fused [RHS at interior + radiation at outer] + RK combine, then inner fill of
 // the array written by that stage.
 cudaError_t hrk_substep(const hr_solver* s, int stage);
+// the two launches of hrk_substep, separately (hr_profile_step times them one by one)
+cudaError_t hrk_substep_main(const hr_solver* s, int stage);
+cudaError_t hrk_substep_fill(const hr_solver* s, int stage);
 // k = full Alg. 1 l.13-14 evaluation of the current state into ku, kv (N_tot each).
 cudaError_t hrk_eval_rhs(const hr_solver* s, void* ku, void* kv);
 // inner fill (C14) of f (N_tot scalars) / of the pair (fu, fv)

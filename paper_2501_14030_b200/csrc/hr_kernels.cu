@@ -402,13 +402,21 @@ cudaError_t hrk_inner_fill(const hr_solver* s, void* fu, void* fv) {
   return s->p.dtype == HR_F64 ? inner_fill_t<double>(s, fu, fv) : inner_fill_t<float>(s, fu, fv);
 }
 
-cudaError_t hrk_substep(const hr_solver* s, int stage) {
-  cudaError_t e = s->p.dtype == HR_F64 ? dispatch_substep<double>(s, stage, nullptr, nullptr)
-                                       : dispatch_substep<float>(s, stage, nullptr, nullptr);
-  if (e != cudaSuccess) return e;
+cudaError_t hrk_substep_main(const hr_solver* s, int stage) {
+  return s->p.dtype == HR_F64 ? dispatch_substep<double>(s, stage, nullptr, nullptr)
+                              : dispatch_substep<float>(s, stage, nullptr, nullptr);
+}
+
+cudaError_t hrk_substep_fill(const hr_solver* s, int stage) {
   // a3 on the array this stage wrote (bitwise equivalent to filling k, C15)
   void* const* out = (stage == 1 || stage == 3) ? s->a.A : (stage == 2 ? s->a.B : s->a.Y);
   return hrk_inner_fill(s, out[0], out[1]);
+}
+
+cudaError_t hrk_substep(const hr_solver* s, int stage) {
+  cudaError_t e = hrk_substep_main(s, stage);
+  if (e != cudaSuccess) return e;
+  return hrk_substep_fill(s, stage);
 }
 
 cudaError_t hrk_eval_rhs(const hr_solver* s, void* ku, void* kv) {
