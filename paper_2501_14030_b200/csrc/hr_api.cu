@@ -8,6 +8,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <limits>
 #include <new>
@@ -52,7 +53,8 @@ hr_status validate(const hr_params* p) {
     return fail(HR_ERR_UNSUPPORTED, "coord %d unknown", p->coord);
   if (p->dtype != HR_F64 && p->dtype != HR_F32)
     return fail(HR_ERR_UNSUPPORTED, "dtype %d unknown", p->dtype);
-  if (p->variant != 0) return fail(HR_ERR_UNSUPPORTED, "variant %d unknown", p->variant);
+  if (p->variant != 0 && p->variant != 2)
+    return fail(HR_ERR_UNSUPPORTED, "variant %d unknown", p->variant);
   const int ng = p->fd_order / 2;
   for (int a = 0; a < 3; ++a)
     if (p->n[a] < ng)
@@ -107,11 +109,7 @@ Layout make_layout(const hr_params* p) {
   L.off_wvol = take(np * 8);
   L.off_inner_dst = take((size_t)L.n_inner * 4 + 4);
   L.off_inner_src = take((size_t)L.n_inner * 4 + 4);
-  HrGrid g{};
-  g.n0 = p->n[0];
-  g.n1 = p->n[1];
-  g.n2 = p->n[2];
-  L.nblocks = hrk_residual_blocks(g);
+  L.nblocks = hrk_max_partials(p->n, L.ng);
   L.off_partials = take((size_t)L.nblocks * 16);
   L.off_result = take(64);
   L.off_rho = take((size_t)L.T[0] * 8);
@@ -401,6 +399,10 @@ hr_status hr_create(const hr_params* p, void* workspace_dev, size_t workspace_by
   g.n_outer_cols = ng;
   s->n_outer = (int64_t)ng * g.n1 * g.n2;
   s->max_partials = L.nblocks;
+  {
+    const char* zc = std::getenv("HR_TUNE_ZC");  // tuning knob: planes per marching chunk
+    s->plan = hrk_make_plan(p->n, ng, p->coord, zc ? std::atoi(zc) : 0);
+  }
 
   char* base = static_cast<char*>(workspace_dev);
   HrArrays& a = s->a;

@@ -56,8 +56,26 @@ struct HrArrays {
   double* punct;               // n_punctures x 10
 };
 
+// Tile of the marching arrangement (hr_march.cuh): BX threads along i0, BY along i1.
+#ifndef HR_TILE_BX
+#define HR_TILE_BX 32
+#endif
+#ifndef HR_TILE_BY
+#define HR_TILE_BY 8
+#endif
+
+// Launch plan of the marching kernels (hr_march.cuh).
+struct MarchPlan {
+  int ntx, nty, nzc;  // tiles along i0, i1; chunks along i2
+  int zc;             // planes per chunk
+  int n_items;        // ntx * nty * nzc marching CTAs
+  int n_rad_blocks;   // CTAs for the outer points (0 for the residual)
+  int sph;            // 1 = SinhSpherical inner map (theta -> pi - theta under rho -> -rho)
+};
+
 struct hr_solver {
   hr_params p;
+  MarchPlan plan;
   std::vector<hr_puncture> punctures;
   HrGrid g;
   HrArrays a;
@@ -89,5 +107,6 @@ cudaError_t hrk_eval_rhs(const hr_solver* s, void* ku, void* kv);
 cudaError_t hrk_inner_fill(const hr_solver* s, void* fu, void* fv);
 // residual partial sums + final deterministic pass into out2_dev
 cudaError_t hrk_residual(const hr_solver* s, int mode, double* out2_dev);
-int hrk_residual_blocks(const HrGrid& g);
+MarchPlan hrk_make_plan(const int32_t n[3], int ng, int coord, int zc_override);
+int hrk_max_partials(const int32_t n[3], int ng);
 int hrk_launches_per_substep(const hr_solver* s);

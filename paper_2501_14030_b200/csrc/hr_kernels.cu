@@ -51,32 +51,49 @@ struct StepArgs {
 //   2: out = Y + dt/2 k ; ACC += dt/3 k
 //   3: out = Y + dt   k ; ACC += dt/3 k
 //   4: Y   = ACC + dt/6 k
+// (yu, yv) = Y and (au, av) = ACC at this point, loaded by the caller where the stage needs them;
+// (wu, wv) returns what was stored to out (the value the point's ghost images take, C15).
 template <typename T, int STAGE>
-__device__ __forceinline__ void rk_combine(const StepArgs<T>& a, int64_t c, T ku, T kv, T in_u,
-                                           T in_v) {
+__device__ __forceinline__ void rk_combine_regs(const StepArgs<T>& a, int64_t c, T ku, T kv, T in_u,
+                                                T in_v, T yu, T yv, T au, T av, T& wu, T& wv) {
   if constexpr (STAGE == 0) {
-    a.out_u[c] = ku;
-    a.out_v[c] = kv;
+    wu = ku;
+    wv = kv;
   } else if constexpr (STAGE == 1) {
     const T h = a.dt * T(0.5), s = a.dt / T(6);
-    a.out_u[c] = in_u + h * ku;
-    a.out_v[c] = in_v + h * kv;
+    wu = in_u + h * ku;
+    wv = in_v + h * kv;
     a.acc_u[c] = in_u + s * ku;
     a.acc_v[c] = in_v + s * kv;
   } else if constexpr (STAGE == 2 || STAGE == 3) {
     const T h = (STAGE == 2) ? a.dt * T(0.5) : a.dt;
     const T s = a.dt / T(3);
-    const T yu = a.y_u[c], yv = a.y_v[c];
-    const T au = a.acc_u[c], av = a.acc_v[c];
-    a.out_u[c] = yu + h * ku;
-    a.out_v[c] = yv + h * kv;
+    wu = yu + h * ku;
+    wv = yv + h * kv;
     a.acc_u[c] = au + s * ku;
     a.acc_v[c] = av + s * kv;
   } else {
     const T s = a.dt / T(6);
-    a.out_u[c] = a.acc_u[c] + s * ku;
-    a.out_v[c] = a.acc_v[c] + s * kv;
+    wu = au + s * ku;
+    wv = av + s * kv;
   }
+  a.out_u[c] = wu;
+  a.out_v[c] = wv;
+}
+
+template <typename T, int STAGE>
+__device__ __forceinline__ void rk_combine(const StepArgs<T>& a, int64_t c, T ku, T kv, T in_u,
+                                           T in_v, T& wu, T& wv) {
+  T yu = T(0), yv = T(0), au = T(0), av = T(0);
+  if constexpr (STAGE == 2 || STAGE == 3) {
+    yu = a.y_u[c];
+    yv = a.y_v[c];
+  }
+  if constexpr (STAGE >= 2) {
+    au = a.acc_u[c];
+    av = a.acc_v[c];
+  }
+  rk_combine_regs<T, STAGE>(a, c, ku, kv, in_u, in_v, yu, yv, au, av, wu, wv);
 }
 
 // Expanded curvilinear Laplacian (C4, C11, C12) with direct global loads of the stencil.
@@ -138,7 +155,8 @@ __global__ void __launch_bounds__(DBX* DBY)
     ku = radiation_k(a.in_u, c, g.s1, r0, r1, ri);
     kv = radiation_k(a.in_v, c, g.s1, r0, r1, ri);
   }
-  rk_combine<T, STAGE>(a, c, ku, kv, uc, vc);
+  T wu, wv;
+  rk_combine<T, STAGE>(a, c, ku, kv, uc, vc, wu, wv);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -286,6 +304,9 @@ __global__ void __launch_bounds__(256)
   S_out[c] = (T)Sval;
 }
 
+
+#include "hr_march.cuh"
+
 // ------------------------------------------------------------------------------------------
 // host-side dispatch
 // ------------------------------------------------------------------------------------------
@@ -307,8 +328,11 @@ StepArgs<T> make_args(const hr_solver* s, int stage, void* ku, void* kv) {
     case 3:
       r.in_u = P(a.B[0]); r.in_v = P(a.B[1]); r.out_u = P(a.A[0]); r.out_v = P(a.A[1]);
       break;
-    default:
+    case 4:
       r.in_u = P(a.A[0]); r.in_v = P(a.A[1]); r.out_u = P(a.Y[0]); r.out_v = P(a.Y[1]);
+      break;
+    default:  // 5, residual: the stencil source is the state
+      r.in_u = P(a.Y[0]); r.in_v = P(a.Y[1]);
       break;
   }
   r.y_u = P(a.Y[0]); r.y_v = P(a.Y[1]);
@@ -321,6 +345,7 @@ StepArgs<T> make_args(const hr_solver* s, int stage, void* ku, void* kv) {
   return r;
 }
 
+// ---- direct-load arrangement (variant 2) ----
 template <typename T, int NG>
 cudaError_t launch_substep_direct(const hr_solver* s, int stage, void* ku, void* kv) {
   const HrGrid& g = s->g;
@@ -337,15 +362,54 @@ cudaError_t launch_substep_direct(const hr_solver* s, int stage, void* ku, void*
   return cudaGetLastError();
 }
 
+// ---- marching arrangement (variant 0) ----
+template <typename T, int NG, int BX, int BY>
+cudaError_t launch_march_tile(const hr_solver* s, int stage, void* ku, void* kv, int mode,
+                              double* partials) {
+  const HrGrid& g = s->g;
+  const StepArgs<T> a = make_args<T>(s, stage, ku, kv);
+  MarchPlan plan = s->plan;
+  ResidArgs ra{s->a.Wvol, partials, mode};
+  if (stage == 5) plan.n_rad_blocks = 0;
+  const dim3 block(BX, BY, 1);
+  const dim3 grid(plan.n_items + plan.n_rad_blocks, 1, 1);
+  switch (stage) {
+    case 0: k_march<T, NG, 0, BX, BY><<<grid, block, 0, s->stream>>>(g, a, plan, ra); break;
+    case 1: k_march<T, NG, 1, BX, BY><<<grid, block, 0, s->stream>>>(g, a, plan, ra); break;
+    case 2: k_march<T, NG, 2, BX, BY><<<grid, block, 0, s->stream>>>(g, a, plan, ra); break;
+    case 3: k_march<T, NG, 3, BX, BY><<<grid, block, 0, s->stream>>>(g, a, plan, ra); break;
+    case 4: k_march<T, NG, 4, BX, BY><<<grid, block, 0, s->stream>>>(g, a, plan, ra); break;
+    default: k_march<T, NG, 5, BX, BY><<<grid, block, 0, s->stream>>>(g, a, plan, ra); break;
+  }
+  return cudaGetLastError();
+}
+
+template <typename T, int NG>
+cudaError_t launch_march(const hr_solver* s, int stage, void* ku, void* kv, int mode,
+                         double* partials) {
+  return launch_march_tile<T, NG, HR_TILE_BX, HR_TILE_BY>(s, stage, ku, kv, mode, partials);
+}
+
 template <typename T>
 cudaError_t dispatch_substep(const hr_solver* s, int stage, void* ku, void* kv) {
+  if (s->p.variant == 2) {
+    switch (s->g.ng) {
+      case 1: return launch_substep_direct<T, 1>(s, stage, ku, kv);
+      case 2: return launch_substep_direct<T, 2>(s, stage, ku, kv);
+      case 3: return launch_substep_direct<T, 3>(s, stage, ku, kv);
+      case 4: return launch_substep_direct<T, 4>(s, stage, ku, kv);
+      case 5: return launch_substep_direct<T, 5>(s, stage, ku, kv);
+      case 6: return launch_substep_direct<T, 6>(s, stage, ku, kv);
+    }
+    return cudaErrorInvalidValue;
+  }
   switch (s->g.ng) {
-    case 1: return launch_substep_direct<T, 1>(s, stage, ku, kv);
-    case 2: return launch_substep_direct<T, 2>(s, stage, ku, kv);
-    case 3: return launch_substep_direct<T, 3>(s, stage, ku, kv);
-    case 4: return launch_substep_direct<T, 4>(s, stage, ku, kv);
-    case 5: return launch_substep_direct<T, 5>(s, stage, ku, kv);
-    case 6: return launch_substep_direct<T, 6>(s, stage, ku, kv);
+    case 1: return launch_march<T, 1>(s, stage, ku, kv, 0, nullptr);
+    case 2: return launch_march<T, 2>(s, stage, ku, kv, 0, nullptr);
+    case 3: return launch_march<T, 3>(s, stage, ku, kv, 0, nullptr);
+    case 4: return launch_march<T, 4>(s, stage, ku, kv, 0, nullptr);
+    case 5: return launch_march<T, 5>(s, stage, ku, kv, 0, nullptr);
+    case 6: return launch_march<T, 6>(s, stage, ku, kv, 0, nullptr);
   }
   return cudaErrorInvalidValue;
 }
@@ -364,15 +428,22 @@ template <typename T, int NG>
 cudaError_t launch_residual(const hr_solver* s, int mode, double* out2) {
   const HrGrid& g = s->g;
   const HrArrays& a = s->a;
-  auto P = [](void* p) { return static_cast<const T*>(p); };
-  const dim3 block(RBX, RBY, 1);
-  const dim3 grid((g.n0 + RBX - 1) / RBX, (g.n1 + RBY - 1) / RBY, g.n2);
-  k_residual<T, NG><<<grid, block, 0, s->stream>>>(g, P(a.Y[0]), P(a.psi), P(a.S), P(a.L00),
-                                                    P(a.L11), P(a.L22), P(a.L0), P(a.L1), a.Wvol,
-                                                    mode, a.partials);
-  cudaError_t e = cudaGetLastError();
+  int64_t nb;
+  cudaError_t e;
+  if (s->p.variant == 2) {
+    auto P = [](void* p) { return static_cast<const T*>(p); };
+    const dim3 block(RBX, RBY, 1);
+    const dim3 grid((g.n0 + RBX - 1) / RBX, (g.n1 + RBY - 1) / RBY, g.n2);
+    k_residual<T, NG><<<grid, block, 0, s->stream>>>(g, P(a.Y[0]), P(a.psi), P(a.S), P(a.L00),
+                                                      P(a.L11), P(a.L22), P(a.L0), P(a.L1), a.Wvol,
+                                                      mode, a.partials);
+    e = cudaGetLastError();
+    nb = (int64_t)grid.x * grid.y * grid.z;
+  } else {
+    e = launch_march<T, NG>(s, 5, nullptr, nullptr, mode, a.partials);
+    nb = s->plan.n_items;
+  }
   if (e != cudaSuccess) return e;
-  const int64_t nb = (int64_t)grid.x * grid.y * grid.z;
   k_residual_final<<<1, 1024, 0, s->stream>>>(a.partials, nb, out2);
   return cudaGetLastError();
 }
@@ -392,11 +463,42 @@ cudaError_t dispatch_residual(const hr_solver* s, int mode, double* out2) {
 
 }  // namespace
 
-int hrk_residual_blocks(const HrGrid& g) {
-  return ((g.n0 + RBX - 1) / RBX) * ((g.n1 + RBY - 1) / RBY) * g.n2;
+// Marching plan for a grid: tile counts and the i2 chunk length.  Enough CTAs to fill the 148
+// SMs several times over, chunks not shorter than the pipeline they have to prime.
+MarchPlan hrk_make_plan(const int32_t n[3], int ng, int coord, int zc_override) {
+  MarchPlan m{};
+  m.ntx = (n[0] + HR_TILE_BX - 1) / HR_TILE_BX;
+  m.nty = (n[1] + HR_TILE_BY - 1) / HR_TILE_BY;
+  const int xy = m.ntx * m.nty;
+  const int target = 148 * 8;
+  int nzc = (target + xy - 1) / xy;
+  const int min_zc = 2 * ng > 8 ? 2 * ng : 8;
+  int max_nzc = n[2] / min_zc;
+  if (max_nzc < 1) max_nzc = 1;
+  if (nzc > max_nzc) nzc = max_nzc;
+  if (nzc < 1) nzc = 1;
+  m.zc = (n[2] + nzc - 1) / nzc;
+  if (zc_override > 0) m.zc = zc_override < n[2] ? zc_override : n[2];
+  m.nzc = (n[2] + m.zc - 1) / m.zc;
+  m.n_items = xy * m.nzc;
+  const int64_t n_outer = (int64_t)ng * n[1] * n[2];
+  m.n_rad_blocks = (int)((n_outer + HR_TILE_BX * HR_TILE_BY - 1) / (HR_TILE_BX * HR_TILE_BY));
+  m.sph = coord == HR_SINHSPHERICAL ? 1 : 0;
+  return m;
 }
 
-int hrk_launches_per_substep(const hr_solver* s) { return s->g.n_inner > 0 ? 2 : 1; }
+int hrk_max_partials(const int32_t n[3], int ng) {
+  const int direct = ((n[0] + RBX - 1) / RBX) * ((n[1] + RBY - 1) / RBY) * n[2];
+  // the marching plan never has more CTAs than one per (tile, plane)
+  const int march = ((n[0] + HR_TILE_BX - 1) / HR_TILE_BX) * ((n[1] + HR_TILE_BY - 1) / HR_TILE_BY) * n[2];
+  (void)ng;
+  return direct > march ? direct : march;
+}
+
+int hrk_launches_per_substep(const hr_solver* s) {
+  if (s->p.variant == 2) return s->g.n_inner > 0 ? 2 : 1;
+  return 1;
+}
 
 cudaError_t hrk_inner_fill(const hr_solver* s, void* fu, void* fv) {
   return s->p.dtype == HR_F64 ? inner_fill_t<double>(s, fu, fv) : inner_fill_t<float>(s, fu, fv);
@@ -408,6 +510,7 @@ cudaError_t hrk_substep_main(const hr_solver* s, int stage) {
 }
 
 cudaError_t hrk_substep_fill(const hr_solver* s, int stage) {
+  if (s->p.variant != 2) return cudaSuccess;  // the marching kernel writes the ghost images itself
   // a3 on the array this stage wrote (bitwise equivalent to filling k, C15)
   void* const* out = (stage == 1 || stage == 3) ? s->a.A : (stage == 2 ? s->a.B : s->a.Y);
   return hrk_inner_fill(s, out[0], out[1]);
@@ -423,6 +526,7 @@ cudaError_t hrk_eval_rhs(const hr_solver* s, void* ku, void* kv) {
   cudaError_t e = s->p.dtype == HR_F64 ? dispatch_substep<double>(s, 0, ku, kv)
                                        : dispatch_substep<float>(s, 0, ku, kv);
   if (e != cudaSuccess) return e;
+  if (s->p.variant != 2) return cudaSuccess;
   return hrk_inner_fill(s, ku, kv);
 }
 

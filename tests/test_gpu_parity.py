@@ -205,7 +205,7 @@ def test_fp32_residual_history_against_fp64_oracle(hr):
     z = np.zeros(o.ntot)
     ou, ov = z.copy(), z.copy()
     ou32, ov32 = z.astype(np.float32), z.astype(np.float32)
-    peak = 0.0
+    peak = o.residual(z, 1)  # C21: the scale is max over n <= N of r_or64(n), n = 0 (u = 0) included
     for it in range(6):
         s32.hr_step(100)
         s64.hr_step(100)
