@@ -399,10 +399,9 @@ hr_status hr_create(const hr_params* p, void* workspace_dev, size_t workspace_by
   g.n_outer_cols = ng;
   s->n_outer = (int64_t)ng * g.n1 * g.n2;
   s->max_partials = L.nblocks;
-  {
-    const char* zc = std::getenv("HR_TUNE_ZC");  // tuning knob: planes per marching chunk
-    s->plan = hrk_make_plan(p->n, ng, p->coord, zc ? std::atoi(zc) : 0);
-  }
+  s->plan = hrk_make_plan(p->n, ng, p->coord);
+  HR_CUDA(cudaDeviceGetAttribute(&s->num_sms, cudaDevAttrMultiProcessorCount, p->device));
+  HR_CUDA(hrk_prepare(s));
 
   char* base = static_cast<char*>(workspace_dev);
   HrArrays& a = s->a;

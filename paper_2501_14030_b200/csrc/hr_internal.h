@@ -64,18 +64,34 @@ struct HrArrays {
 #define HR_TILE_BY 8
 #endif
 
-// Launch plan of the marching kernels (hr_march.cuh).
+// Minimum resident CTAs per SM the marching kernels are compiled for (register cap).
+#ifndef HR_MARCH_MINB_F64
+#define HR_MARCH_MINB_F64 2
+#endif
+#ifndef HR_MARCH_MINB_F32
+#define HR_MARCH_MINB_F32 3
+#endif
+
+// Planes of asynchronous look-ahead in the marching kernels.
+#ifndef HR_MARCH_D_F64
+#define HR_MARCH_D_F64 2
+#endif
+#ifndef HR_MARCH_D_F32
+#define HR_MARCH_D_F32 3
+#endif
+
+// Tiling of the marching kernels (hr_march.cuh).
 struct MarchPlan {
-  int ntx, nty, nzc;  // tiles along i0, i1; chunks along i2
-  int zc;             // planes per chunk
-  int n_items;        // ntx * nty * nzc marching CTAs
-  int n_rad_blocks;   // CTAs for the outer points (0 for the residual)
-  int sph;            // 1 = SinhSpherical inner map (theta -> pi - theta under rho -> -rho)
+  int ntx, nty;  // tiles along i0, i1
+  int zc, nzc;   // planes per chunk, chunks along i2
+  int sph;       // 1 = SinhSpherical inner map (theta -> pi - theta under rho -> -rho)
 };
 
 struct hr_solver {
   hr_params p;
   MarchPlan plan;
+  int num_sms;
+  int march_grid[6];  // persistent grid size per stage kernel (0 = eval, 1..4, 5 = residual)
   std::vector<hr_puncture> punctures;
   HrGrid g;
   HrArrays a;
@@ -107,6 +123,8 @@ cudaError_t hrk_eval_rhs(const hr_solver* s, void* ku, void* kv);
 cudaError_t hrk_inner_fill(const hr_solver* s, void* fu, void* fv);
 // residual partial sums + final deterministic pass into out2_dev
 cudaError_t hrk_residual(const hr_solver* s, int mode, double* out2_dev);
-MarchPlan hrk_make_plan(const int32_t n[3], int ng, int coord, int zc_override);
+MarchPlan hrk_make_plan(const int32_t n[3], int ng, int coord);
+// shared-memory opt-in and persistent grid sizes of the marching kernels; before graph capture
+cudaError_t hrk_prepare(hr_solver* s);
 int hrk_max_partials(const int32_t n[3], int ng);
 int hrk_launches_per_substep(const hr_solver* s);

