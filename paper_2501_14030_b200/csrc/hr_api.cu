@@ -43,7 +43,7 @@ hr_status fail(hr_status st, const char* fmt, ...) {
 
 constexpr double kPi = 3.141592653589793238462643383279502884;
 
-size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+size_t align_up(size_t x, size_t a = 1024) { return (x + a - 1) / a * a; }
 
 hr_status validate(const hr_params* p) {
   if (!p) return fail(HR_ERR_INVALID_ARG, "params is NULL");
@@ -61,7 +61,8 @@ hr_status validate(const hr_params* p) {
       return fail(HR_ERR_INVALID_ARG, "n[%d] = %d is smaller than NG = %d", a, p->n[a], ng);
   if (p->n[2] % 2) return fail(HR_ERR_INVALID_ARG, "n[2] = %d must be even (C14)", p->n[2]);
   const double tot = double(p->n[0] + 2 * ng) * double(p->n[1] + 2 * ng) * double(p->n[2] + 2 * ng);
-  if (tot >= 2147483647.0) return fail(HR_ERR_INVALID_ARG, "grid exceeds int32 index range");
+  if (tot * 1.25 + 1e6 >= 2147483647.0)
+    return fail(HR_ERR_INVALID_ARG, "grid exceeds int32 index range");
   if (!(p->amp > 0) || !(p->sinhw > 0)) return fail(HR_ERR_INVALID_ARG, "amp, sinhw must be > 0");
   if (p->coord == HR_SINHSYMTP && !(p->bscale > 0))
     return fail(HR_ERR_INVALID_ARG, "bscale must be > 0 for SinhSymTP");
@@ -84,8 +85,8 @@ struct Layout {
   size_t off_wvol, off_inner_dst, off_inner_src, off_partials, off_result;
   size_t off_rho, off_rhoz, off_sinth, off_costh, off_sinph, off_cosph, off_punct;
   size_t total;
-  int64_t ntot, n_inner;
-  int T[3], ng;
+  int64_t ntot, n_inner, npad;
+  int T[3], ng, P0, off0;
   int nblocks;
 };
 
@@ -96,13 +97,15 @@ Layout make_layout(const hr_params* p) {
   L.ntot = (int64_t)L.T[0] * L.T[1] * L.T[2];
   L.n_inner = L.ntot - (int64_t)p->n[0] * p->n[1] * p->n[2] - (int64_t)L.ng * p->n[1] * p->n[2];
   const size_t w = p->dtype == HR_F64 ? 8 : 4;
+  hrk_row_geometry(L.T[0], L.ng, w, &L.P0, &L.off0);
+  L.npad = (int64_t)L.P0 * L.T[1] * L.T[2];
   size_t off = 0;
   auto take = [&](size_t bytes) {
     size_t o = off;
     off = align_up(off + bytes);
     return o;
   };
-  for (int f = 0; f < 10; ++f) L.off_field[f] = take((size_t)L.ntot * w);
+  for (int f = 0; f < 10; ++f) L.off_field[f] = take((size_t)L.npad * w);
   const size_t np = (size_t)L.T[0] * L.T[1];
   for (int f = 0; f < 6; ++f) L.off_plane[f] = take(np * w);
   for (int f = 0; f < 3; ++f) L.off_rad[f] = take((size_t)L.ng * L.T[1] * w);
@@ -392,8 +395,11 @@ hr_status hr_create(const hr_params* p, void* workspace_dev, size_t workspace_by
   g.n0 = p->n[0]; g.n1 = p->n[1]; g.n2 = p->n[2];
   g.ng = ng;
   g.T0 = L.T[0]; g.T1 = L.T[1]; g.T2 = L.T[2];
-  g.s1 = g.T0;
-  g.s2 = (int64_t)g.T0 * g.T1;
+  g.P0 = L.P0;
+  g.off0 = L.off0;
+  g.s1 = g.P0;
+  g.s2 = (int64_t)g.P0 * g.T1;
+  g.npad = L.npad;
   g.ntot = L.ntot;
   g.n_inner = L.n_inner;
   g.n_outer_cols = ng;
@@ -448,8 +454,20 @@ hr_status hr_create(const hr_params* p, void* workspace_dev, size_t workspace_by
   HR_TRY(upload_plane(s, a.RAD1, H.r1));
   HR_TRY(upload_plane(s, a.RADI, H.ri));
   HR_TRY(upload(a.Wvol, H.wv.data(), np * 8, s->stream));
-  HR_TRY(upload(a.inner_dst, s->inner_dst.data(), s->inner_dst.size() * 4, s->stream));
-  HR_TRY(upload(a.inner_src, s->inner_src.data(), s->inner_src.size() * 4, s->stream));
+  {
+    // device copies of the inner lists in stored (padded) indices; the host copies stay public
+    auto stored = [&](const std::vector<int32_t>& v) {
+      std::vector<int32_t> r(v.size());
+      for (size_t i = 0; i < v.size(); ++i) {
+        const int32_t row = v[i] / g.T0;
+        r[i] = g.off0 + (v[i] - row * g.T0) + g.P0 * row;
+      }
+      return r;
+    };
+    const std::vector<int32_t> d = stored(s->inner_dst), sr = stored(s->inner_src);
+    HR_TRY(upload(a.inner_dst, d.data(), d.size() * 4, s->stream));
+    HR_TRY(upload(a.inner_src, sr.data(), sr.size() * 4, s->stream));
+  }
   HR_TRY(upload(a.rho, H.rho.data(), H.rho.size() * 8, s->stream));
   HR_TRY(upload(a.rhoz, H.rhoz.data(), H.rhoz.size() * 8, s->stream));
   HR_TRY(upload(a.sinth, H.sth.data(), H.sth.size() * 8, s->stream));
@@ -460,8 +478,8 @@ hr_status hr_create(const hr_params* p, void* workspace_dev, size_t workspace_by
   HR_TRY(upload(a.punct, s->punctures.data(), s->punctures.size() * sizeof(hr_puncture), s->stream));
 
   // ---- Alg. 1 l.5, 7: zero state (C17) and constant source terms on the device ----
-  const size_t fb = (size_t)g.ntot * s->scalar_bytes;
-  for (void* f : {a.Y[0], a.Y[1], a.A[0], a.A[1], a.B[0], a.B[1], a.ACC[0], a.ACC[1]})
+  const size_t fb = (size_t)g.npad * s->scalar_bytes;
+  for (void* f : {a.Y[0], a.Y[1], a.A[0], a.A[1], a.B[0], a.B[1], a.ACC[0], a.ACC[1], a.psi, a.S})
     HR_CUDA(cudaMemsetAsync(f, 0, fb, s->stream));
   HR_CUDA(hrk_source(s));
   int bad = 0;
@@ -566,12 +584,18 @@ hr_status hr_residual(hr_solver* s, double* out) {
   return st;
 }
 
+// Copy one stored grid function out in the public layout.  A (stage buffer, free between steps)
+// is the device staging area for host destinations.
 static hr_status get_field(hr_solver* s, const void* src, void* dst, size_t bytes, int on_device) {
   if (!s || !dst) return fail(HR_ERR_INVALID_ARG, "NULL argument");
   const size_t need = (size_t)s->g.ntot * s->scalar_bytes;
   if (bytes != need) return fail(HR_ERR_INVALID_ARG, "bytes = %zu, expected %zu", bytes, need);
-  HR_CUDA(cudaMemcpyAsync(dst, src, need, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost,
-                          s->stream));
+  if (on_device) {
+    HR_CUDA(hrk_pack(s, dst, src));
+  } else {
+    HR_CUDA(hrk_pack(s, s->a.A[0], src));
+    HR_CUDA(cudaMemcpyAsync(dst, s->a.A[0], need, cudaMemcpyDeviceToHost, s->stream));
+  }
   HR_CUDA(cudaStreamSynchronize(s->stream));
   return HR_OK;
 }
@@ -587,9 +611,15 @@ hr_status hr_get_v(hr_solver* s, void* dst, size_t bytes, int32_t dst_on_device)
 hr_status hr_set_state(hr_solver* s, const void* u, const void* v, int32_t src_on_device) {
   if (!s || !u || !v) return fail(HR_ERR_INVALID_ARG, "NULL argument");
   const size_t need = (size_t)s->g.ntot * s->scalar_bytes;
-  const cudaMemcpyKind kind = src_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
-  HR_CUDA(cudaMemcpyAsync(s->a.Y[0], u, need, kind, s->stream));
-  HR_CUDA(cudaMemcpyAsync(s->a.Y[1], v, need, kind, s->stream));
+  if (src_on_device) {
+    HR_CUDA(hrk_unpack(s, s->a.Y[0], u));
+    HR_CUDA(hrk_unpack(s, s->a.Y[1], v));
+  } else {
+    HR_CUDA(cudaMemcpyAsync(s->a.A[0], u, need, cudaMemcpyHostToDevice, s->stream));
+    HR_CUDA(cudaMemcpyAsync(s->a.A[1], v, need, cudaMemcpyHostToDevice, s->stream));
+    HR_CUDA(hrk_unpack(s, s->a.Y[0], s->a.A[0]));
+    HR_CUDA(hrk_unpack(s, s->a.Y[1], s->a.A[1]));
+  }
   HR_CUDA(hrk_inner_fill(s, s->a.Y[0], s->a.Y[1]));
   if (!src_on_device) HR_CUDA(cudaStreamSynchronize(s->stream));
   return HR_OK;
@@ -597,15 +627,24 @@ hr_status hr_set_state(hr_solver* s, const void* u, const void* v, int32_t src_o
 
 hr_status hr_eval_rhs(hr_solver* s, void* ku_dev, void* kv_dev) {
   if (!s || !ku_dev || !kv_dev) return fail(HR_ERR_INVALID_ARG, "NULL argument");
-  HR_CUDA(hrk_eval_rhs(s, ku_dev, kv_dev));
+  // k is produced in the stored layout in B (free between steps), then packed out
+  HR_CUDA(hrk_eval_rhs(s, s->a.B[0], s->a.B[1]));
+  HR_CUDA(hrk_pack(s, ku_dev, s->a.B[0]));
+  HR_CUDA(hrk_pack(s, kv_dev, s->a.B[1]));
   return HR_OK;
 }
 
 hr_status hr_get_source(hr_solver* s, void* psi_host, void* S_host) {
   if (!s) return fail(HR_ERR_INVALID_ARG, "solver is NULL");
   const size_t need = (size_t)s->g.ntot * s->scalar_bytes;
-  if (psi_host) HR_CUDA(cudaMemcpyAsync(psi_host, s->a.psi, need, cudaMemcpyDeviceToHost, s->stream));
-  if (S_host) HR_CUDA(cudaMemcpyAsync(S_host, s->a.S, need, cudaMemcpyDeviceToHost, s->stream));
+  if (psi_host) {
+    HR_CUDA(hrk_pack(s, s->a.A[0], s->a.psi));
+    HR_CUDA(cudaMemcpyAsync(psi_host, s->a.A[0], need, cudaMemcpyDeviceToHost, s->stream));
+  }
+  if (S_host) {
+    HR_CUDA(hrk_pack(s, s->a.A[1], s->a.S));
+    HR_CUDA(cudaMemcpyAsync(S_host, s->a.A[1], need, cudaMemcpyDeviceToHost, s->stream));
+  }
   HR_CUDA(cudaStreamSynchronize(s->stream));
   return HR_OK;
 }

@@ -13,12 +13,19 @@
 #define HR_MAX_NG 6
 
 // Device-side view of one solver: everything a kernel needs, passed by value (__grid_constant__).
-// Grid functions are stored with the public layout idx = i0 + T0 (i1 + T1 i2) (reading C8).
+// The PUBLIC layout of a grid function is idx = i0 + T0 (i1 + T1 i2) (reading C8).  In HBM the
+// library keeps a padded copy of that layout: point (i0,i1,i2) sits at
+//     off0 + i0 + P0 (i1 + T1 i2),   P0 = row pitch >= off0 + T0,
+// with P0 and off0 + NG multiples of 128 bytes, so that the first interior point of every row
+// starts a 128-byte line (full-sector warp stores, aligned vector loads, TMA-legal strides).
+// hr_get_u / hr_set_state / hr_eval_rhs convert between the two with k_pack / k_unpack.
 struct HrGrid {
   int32_t n0, n1, n2;  // interior points
   int32_t ng;          // ghost layers = FD radius (C7)
   int32_t T0, T1, T2;  // points per axis incl. ghosts
-  int64_t s1, s2;      // strides of i1 and i2 in scalars (T0, T0*T1)
+  int32_t P0, off0;    // padded row pitch and offset of i0 = 0 within a row, in scalars
+  int64_t s1, s2;      // strides of i1 and i2 in scalars (P0, P0*T1)
+  int64_t npad;        // scalars per stored grid function (P0*T1*T2)
   int64_t ntot;
   int64_t n_inner;
   int32_t n_outer_cols;  // = ng: outer layers i0 in [n0+ng, T0)
@@ -119,8 +126,13 @@ cudaError_t hrk_substep_main(const hr_solver* s, int stage);
 cudaError_t hrk_substep_fill(const hr_solver* s, int stage);
 // k = full Alg. 1 l.13-14 evaluation of the current state into ku, kv (N_tot each).
 cudaError_t hrk_eval_rhs(const hr_solver* s, void* ku, void* kv);
-// inner fill (C14) of f (N_tot scalars) / of the pair (fu, fv)
+// inner fill (C14) of the pair (fu, fv), stored layout
 cudaError_t hrk_inner_fill(const hr_solver* s, void* fu, void* fv);
+// public layout (N_tot scalars, device) <-> stored layout
+cudaError_t hrk_pack(const hr_solver* s, void* dst_public, const void* src_stored);
+cudaError_t hrk_unpack(const hr_solver* s, void* dst_stored, const void* src_public);
+// padded row geometry for a dtype: pitch and offset in scalars
+void hrk_row_geometry(int T0, int ng, size_t scalar_bytes, int* P0, int* off0);
 // residual partial sums + final deterministic pass into out2_dev
 cudaError_t hrk_residual(const hr_solver* s, int mode, double* out2_dev);
 MarchPlan hrk_make_plan(const int32_t n[3], int ng, int coord);

@@ -142,7 +142,7 @@ __global__ void __launch_bounds__(DBX* DBY)
   const int i1 = NG + blockIdx.y * DBY + threadIdx.y;
   const int i2 = NG + blockIdx.z;
   if (i0 >= g.T0 || i1 >= g.n1 + NG) return;
-  const int64_t c = i0 + g.s1 * i1 + g.s2 * i2;
+  const int64_t c = g.off0 + i0 + g.s1 * i1 + g.s2 * i2;
   const T uc = a.in_u[c], vc = a.in_v[c];
   T ku, kv;
   if (i0 < g.n0 + NG) {
@@ -192,7 +192,7 @@ __global__ void __launch_bounds__(RBX* RBY)
   const int i2 = NG + blockIdx.z;
   double num = 0.0, den = 0.0;
   if (i0 < g.n0 + NG && i1 < g.n1 + NG) {
-    const int64_t c = i0 + g.s1 * i1 + g.s2 * i2;
+    const int64_t c = g.off0 + i0 + g.s1 * i1 + g.s2 * i2;
     const int64_t q = i0 + (int64_t)g.T0 * i1;
     const T uc = u[c];
     const T lap =
@@ -267,7 +267,8 @@ __global__ void __launch_bounds__(256)
   if (c >= g.ntot) return;
   const int i0 = (int)(c % g.T0);
   const int i1 = (int)((c / g.T0) % g.T1);
-  const int i2 = (int)(c / g.s2);
+  const int i2 = (int)(c / ((int64_t)g.T0 * g.T1));
+  const int64_t cs = g.off0 + i0 + g.s1 * i1 + g.s2 * i2;  // stored index
   // grid point in Cartesian coordinates (C4) + grid centre (C6)
   const double rs = rho[i0] * sinth[i1];
   const double x = rs * cosph[i2] + ox;
@@ -302,8 +303,25 @@ __global__ void __launch_bounds__(256)
   const double AA = axx * axx + ayy * ayy + azz * azz + 2.0 * (axy * axy + axz * axz + ayz * ayz);
   const double Sval = 0.125 * AA;
   if (!isfinite(psi) || !isfinite(Sval)) atomicOr(bad_flag, 1);
-  psi_out[c] = (T)psi;
-  S_out[c] = (T)Sval;
+  psi_out[cs] = (T)psi;
+  S_out[cs] = (T)Sval;
+}
+
+// ------------------------------------------------------------------------------------------
+// public layout <-> stored (padded) layout
+// ------------------------------------------------------------------------------------------
+template <typename T, bool TO_PUBLIC>
+__global__ void __launch_bounds__(256)
+    k_repack(const __grid_constant__ HrGrid g, T* __restrict__ dst, const T* __restrict__ src) {
+  const int i0 = blockIdx.y * 256 + threadIdx.x;
+  if (i0 >= g.T0) return;
+  const int64_t row = blockIdx.x;  // i1 + T1 i2
+  const int64_t pub = i0 + (int64_t)g.T0 * row;
+  const int64_t sto = g.off0 + i0 + g.s1 * row;
+  if (TO_PUBLIC)
+    dst[pub] = src[sto];
+  else
+    dst[sto] = src[pub];
 }
 
 
@@ -541,6 +559,34 @@ int hrk_max_partials(const int32_t n[3], int ng) {
 int hrk_launches_per_substep(const hr_solver* s) {
   if (s->p.variant == 2) return s->g.n_inner > 0 ? 2 : 1;
   return 1;
+}
+
+void hrk_row_geometry(int T0, int ng, size_t scalar_bytes, int* P0, int* off0) {
+  const int line = (int)(128 / scalar_bytes);  // scalars per 128-byte line
+  const int lead = (ng + line - 1) / line * line;  // first interior point starts a line
+  *off0 = lead - ng;
+  *P0 = (*off0 + T0 + line - 1) / line * line;
+}
+
+template <typename T>
+cudaError_t repack_t(const hr_solver* s, void* dst, const void* src, bool to_public) {
+  const HrGrid& g = s->g;
+  const dim3 grid(g.T1 * g.T2, (g.T0 + 255) / 256, 1);
+  if (to_public)
+    k_repack<T, true><<<grid, 256, 0, s->stream>>>(g, static_cast<T*>(dst), static_cast<const T*>(src));
+  else
+    k_repack<T, false><<<grid, 256, 0, s->stream>>>(g, static_cast<T*>(dst), static_cast<const T*>(src));
+  return cudaGetLastError();
+}
+
+cudaError_t hrk_pack(const hr_solver* s, void* dst_public, const void* src_stored) {
+  return s->p.dtype == HR_F64 ? repack_t<double>(s, dst_public, src_stored, true)
+                              : repack_t<float>(s, dst_public, src_stored, true);
+}
+
+cudaError_t hrk_unpack(const hr_solver* s, void* dst_stored, const void* src_public) {
+  return s->p.dtype == HR_F64 ? repack_t<double>(s, dst_stored, src_public, false)
+                              : repack_t<float>(s, dst_stored, src_public, false);
 }
 
 cudaError_t hrk_inner_fill(const hr_solver* s, void* fu, void* fv) {

@@ -55,7 +55,7 @@ __device__ __forceinline__ void scatter_images(const HrGrid& g, int sph, T* __re
   const int ng = g.ng;
   const int kbase = j2 - ng;
   const int half = g.n2 >> 1;
-  const int s2 = g.T0 * g.T1;
+  const int s2 = g.P0 * g.T1;
 #pragma unroll
   for (int f0 = 0; f0 < 2; ++f0) {
     if (f0 && r0 < 0) continue;
@@ -68,7 +68,7 @@ __device__ __forceinline__ void scatter_images(const HrGrid& g, int sph, T* __re
       const int flips = f0 + (m != 0);
       int kd = kbase - ((flips & 1) ? half : 0);
       if (kd < 0) kd += g.n2;
-      const int base = d0 + g.T0 * d1;
+      const int base = g.off0 + d0 + g.P0 * d1;
       if (f0 || m) {
         const int d = base + (kd + ng) * s2;
         ou[d] = vu;
@@ -123,7 +123,7 @@ __global__ void __launch_bounds__(BX* BY, sizeof(T) == 8 ? HR_MARCH_MINB_F64 : H
 
   const int lx = threadIdx.x, ly = threadIdx.y;
   const int tid = ly * BX + lx;
-  const int s2 = g.T0 * g.T1;
+  const int s2 = g.P0 * g.T1;
   const T* __restrict__ uin = a.in_u;
   const int ctr = (ly + NG) * SW + lx + NG;  // this thread's point in a tile
 
@@ -145,7 +145,7 @@ __global__ void __launch_bounds__(BX* BY, sizeof(T) == 8 ? HR_MARCH_MINB_F64 : H
     const bool active = i0 < g.n0 + NG && i1 < g.n1 + NG;
     // inactive threads of edge tiles still feed the tile centre (their points are ghosts that
     // the neighbours' stencils read), so they track real grid values, clamped to the grid
-    const int col = min(i0, g.T0 - 1) + g.T0 * min(i1, g.T1 - 1);
+    const int col = g.off0 + min(i0, g.T0 - 1) + g.P0 * min(i1, g.T1 - 1);
 
     // halo ring slots of this thread: tile offset and in-plane global offset (-1: none)
     int h_s[NSLOT], h_g[NSLOT];
@@ -165,7 +165,7 @@ __global__ void __launch_bounds__(BX* BY, sizeof(T) == 8 ? HR_MARCH_MINB_F64 : H
       }
       const int gi0 = tx * BX + c, gi1 = ty * BY + r;
       h_s[s] = r * SW + c;
-      h_g[s] = (h < NHALO && gi0 < g.T0 && gi1 < g.T1) ? gi0 + g.T0 * gi1 : -1;
+      h_g[s] = (h < NHALO && gi0 < g.T0 && gi1 < g.T1) ? g.off0 + gi0 + g.P0 * gi1 : -1;
     }
 
     // per-column constants
@@ -214,73 +214,79 @@ __global__ void __launch_bounds__(BX* BY, sizeof(T) == 8 ? HR_MARCH_MINB_F64 : H
       cp_async_commit();
     };
 
-    // prologue: look-ahead groups, then the register pipeline p[j] = u(i0, i1, z - NG + j)
+    // prologue: look-ahead groups, then the register pipeline.  w(k) = u(i0, i1, z - NG + k),
+    // k = 0..2NG, lives in p[(j + k) % U] where j = (z - z_begin) % U: the plane loop is unrolled
+    // U = 2NG+1 times so the window rotates through the registers without moves.
 #pragma unroll
     for (int d = 0; d < D; ++d) issue(z_begin + d, d);
-    T p[2 * NG + 1];
+    constexpr int U = 2 * NG + 1;
+    T p[U];
 #pragma unroll
-    for (int j = 0; j <= 2 * NG; ++j) p[j] = uin[col + (z_begin - NG + j) * s2];
+    for (int k = 0; k < 2 * NG; ++k) p[k] = uin[col + (z_begin - NG + k) * s2];
     tiles[ctr] = p[NG];
 
     int sl = 0;  // ring slot of plane z
-    for (int z = z_begin; z < z_end; ++z) {
-      cp_async_wait_group<D - 1>();  // this thread's group of plane z has landed
-      __syncthreads();               // everyone's has; slot of plane z-1 is free again
-      {
-        int sn = sl + D;
-        if (sn >= RING) sn -= RING;
-        issue(z + D, sn);
-      }
-      const T* tl = tiles + sl * TILE;
-      const T* st = strm + sl * (NS * NT) + tid;
-      if (z > z_begin) {
+    for (int zb = z_begin; zb < z_end; zb += U) {
 #pragma unroll
-        for (int j = 0; j < 2 * NG; ++j) p[j] = p[j + 1];
-        p[2 * NG] = st[ST_FRONT * NT];
-      }
-      int sn1 = sl + 1;
-      if (sn1 >= RING) sn1 = 0;
-      if (z + 1 < z_end) tiles[sn1 * TILE + ctr] = p[NG + 1];
+      for (int j = 0; j < U; ++j) {
+        const int z = zb + j;
+        if (z >= z_end) break;
+#define HR_W(k) p[(j + (k)) % U]
+        cp_async_wait_group<D - 1>();  // this thread's group of plane z has landed
+        __syncthreads();               // everyone's has; slot of plane z-1 is free again
+        {
+          int sn = sl + D;
+          if (sn >= RING) sn -= RING;
+          issue(z + D, sn);
+        }
+        const T* tl = tiles + sl * TILE;
+        const T* st = strm + sl * (NS * NT) + tid;
+        HR_W(2 * NG) = st[ST_FRONT * NT];
+        int sn1 = sl + 1;
+        if (sn1 >= RING) sn1 = 0;
+        if (z + 1 < z_end) tiles[sn1 * TILE + ctr] = HR_W(NG + 1);
 
-      if (active) {
-        const int c = col + z * s2;
-        const T uc = p[NG];
-        T d00 = T(F::d2(0)) * uc, d11 = d00, d22 = d00, d0 = T(0), d1 = T(0);
+        if (active) {
+          const int c = col + z * s2;
+          const T uc = HR_W(NG);
+          T d00 = T(F::d2(0)) * uc, d11 = d00, d22 = d00, d0 = T(0), d1 = T(0);
 #pragma unroll
-        for (int k = 1; k <= NG; ++k) {
-          const T a0 = tl[ctr + k], b0 = tl[ctr - k];
-          const T a1 = tl[ctr + k * SW], b1 = tl[ctr - k * SW];
-          d00 += T(F::d2(k)) * (a0 + b0);
-          d11 += T(F::d2(k)) * (a1 + b1);
-          d22 += T(F::d2(k)) * (p[NG + k] + p[NG - k]);
-          d0 += T(F::c1(k)) * (a0 - b0);
-          d1 += T(F::c1(k)) * (a1 - b1);
-        }
-        const T lap = l00 * d00 + l11 * d11 + l22 * d22 + l0 * d0 + l1 * d1;
-        const T H = lap + st[ST_S * NT] * pow_m7(st[ST_PSI * NT] + uc);
-        if constexpr (STAGE == 5) {
-          num += wq * (double)H * (double)H;
-          den += wq;
-        } else {
-          const T vc = st[ST_V * NT];
-          T yu = T(0), yv = T(0), au = T(0), av = T(0);
-          if constexpr (STAGE >= 2 && STAGE <= 4) {
-            au = st[ST_AU * NT];
-            av = st[ST_AV * NT];
+          for (int k = 1; k <= NG; ++k) {
+            const T a0 = tl[ctr + k], b0 = tl[ctr - k];
+            const T a1 = tl[ctr + k * SW], b1 = tl[ctr - k * SW];
+            d00 += T(F::d2(k)) * (a0 + b0);
+            d11 += T(F::d2(k)) * (a1 + b1);
+            d22 += T(F::d2(k)) * (HR_W(NG + k) + HR_W(NG - k));
+            d0 += T(F::c1(k)) * (a0 - b0);
+            d1 += T(F::c1(k)) * (a1 - b1);
           }
-          if constexpr (STAGE == 2 || STAGE == 3) {
-            yu = st[ST_YU * NT];
-            yv = st[ST_YV * NT];
+          const T lap = l00 * d00 + l11 * d11 + l22 * d22 + l0 * d0 + l1 * d1;
+          const T H = lap + st[ST_S * NT] * pow_m7(st[ST_PSI * NT] + uc);
+          if constexpr (STAGE == 5) {
+            num += wq * (double)H * (double)H;
+            den += wq;
+          } else {
+            const T vc = st[ST_V * NT];
+            T yu = T(0), yv = T(0), au = T(0), av = T(0);
+            if constexpr (STAGE >= 2 && STAGE <= 4) {
+              au = st[ST_AU * NT];
+              av = st[ST_AV * NT];
+            }
+            if constexpr (STAGE == 2 || STAGE == 3) {
+              yu = st[ST_YU * NT];
+              yv = st[ST_YV * NT];
+            }
+            const T ku = vc - a.eta * uc;
+            const T kv = c2 * H;
+            T wu, wv;
+            rk_combine_regs<T, STAGE>(a, c, ku, kv, uc, vc, yu, yv, au, av, wu, wv);
+            if (inplane_images || z < 2 * NG || z >= g.n2)
+              scatter_images<T>(g, plan.sph, a.out_u, a.out_v, wu, wv, i0, i1, z, r0, cB, cC);
           }
-          const T ku = vc - a.eta * uc;
-          const T kv = c2 * H;
-          T wu, wv;
-          rk_combine_regs<T, STAGE>(a, c, ku, kv, uc, vc, yu, yv, au, av, wu, wv);
-          if (inplane_images || z < 2 * NG || z >= g.n2)
-            scatter_images<T>(g, plan.sph, a.out_u, a.out_v, wu, wv, i0, i1, z, r0, cB, cC);
         }
+        if (++sl >= RING) sl = 0;
+#undef HR_W
       }
-      if (++sl >= RING) sl = 0;
     }
     cp_async_wait_all();
     __syncthreads();  // the ring is reused by the next segment
@@ -316,12 +322,12 @@ __global__ void __launch_bounds__(BX* BY, sizeof(T) == 8 ? HR_MARCH_MINB_F64 : H
       const int r = m / NG;
       const int i1 = NG + r % g.n1, i2 = NG + r / g.n1;
       const int i0 = g.n0 + NG + j;
-      const int c = i0 + g.T0 * i1 + s2 * i2;
+      const int c = g.off0 + i0 + g.P0 * i1 + s2 * i2;
       const int qo = j + NG * i1;
       const T r0 = a.RAD0[qo], r1 = a.RAD1[qo], ri = a.RADI[qo];
       const T uc = a.in_u[c], vc = a.in_v[c];
-      const T ku = radiation_k(a.in_u, c, g.T0, r0, r1, ri);
-      const T kv = radiation_k(a.in_v, c, g.T0, r0, r1, ri);
+      const T ku = radiation_k(a.in_u, c, g.P0, r0, r1, ri);
+      const T kv = radiation_k(a.in_v, c, g.P0, r0, r1, ri);
       T wu, wv;
       rk_combine<T, STAGE>(a, c, ku, kv, uc, vc, wu, wv);
       const int cB = i1 < 2 * NG ? 2 * NG - 1 - i1 : -1;
