@@ -405,9 +405,8 @@ hr_status hr_create(const hr_params* p, void* workspace_dev, size_t workspace_by
   g.n_outer_cols = ng;
   s->n_outer = (int64_t)ng * g.n1 * g.n2;
   s->max_partials = L.nblocks;
-  s->plan = hrk_make_plan(p->n, ng, p->coord);
+  s->plan = hrk_make_plan(p->n, ng, p->coord, p->dtype);
   HR_CUDA(cudaDeviceGetAttribute(&s->num_sms, cudaDevAttrMultiProcessorCount, p->device));
-  HR_CUDA(hrk_prepare(s));
 
   char* base = static_cast<char*>(workspace_dev);
   HrArrays& a = s->a;
@@ -431,6 +430,8 @@ hr_status hr_create(const hr_params* p, void* workspace_dev, size_t workspace_by
   a.sinph = reinterpret_cast<double*>(base + L.off_sinph);
   a.cosph = reinterpret_cast<double*>(base + L.off_cosph);
   a.punct = reinterpret_cast<double*>(base + L.off_punct);
+
+  HR_CUDA(hrk_prepare(s));  // tensor maps, shared-memory opt-in, persistent grid sizes
 
   // ---- Alg. 1 l.2-4 on the host ----
   HostSetup H;

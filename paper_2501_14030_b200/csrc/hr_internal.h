@@ -2,6 +2,7 @@
 // hr_kernels.cu (device code).  Product code: shares nothing with oracle/.
 #pragma once
 
+#include <cuda.h>  // CUtensorMap (types only; the driver is reached through the runtime)
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -63,12 +64,16 @@ struct HrArrays {
   double* punct;               // n_punctures x 10
 };
 
-// Tile of the marching arrangement (hr_march.cuh): BX threads along i0, BY along i1.
-#ifndef HR_TILE_BX
-#define HR_TILE_BX 32
+// Tiles of the marching arrangement (hr_march.cuh): TW x BY points, VX points per thread.
+#ifndef HR_TW_F64
+#define HR_TW_F64 32
+#define HR_BY_F64 8
+#define HR_VX_F64 1
 #endif
-#ifndef HR_TILE_BY
-#define HR_TILE_BY 8
+#ifndef HR_TW_F32
+#define HR_TW_F32 64
+#define HR_BY_F32 8
+#define HR_VX_F32 2
 #endif
 
 // Minimum resident CTAs per SM the marching kernels are compiled for (register cap).
@@ -79,12 +84,17 @@ struct HrArrays {
 #define HR_MARCH_MINB_F32 3
 #endif
 
+// 1: unroll the plane loop 2NG+1 times (rotating register window); 0: single copy + moves.
+#ifndef HR_MARCH_ROTATE
+#define HR_MARCH_ROTATE 1
+#endif
+
 // Planes of asynchronous look-ahead in the marching kernels.
 #ifndef HR_MARCH_D_F64
 #define HR_MARCH_D_F64 2
 #endif
 #ifndef HR_MARCH_D_F32
-#define HR_MARCH_D_F32 3
+#define HR_MARCH_D_F32 2
 #endif
 
 // Tiling of the marching kernels (hr_march.cuh).
@@ -99,6 +109,10 @@ struct hr_solver {
   MarchPlan plan;
   int num_sms;
   int march_grid[6];  // persistent grid size per stage kernel (0 = eval, 1..4, 5 = residual)
+  // TMA descriptors of the ten stored grid functions (Y, A, B, ACC (u, v), psi, S): the TW x BY
+  // box of each, and the halo-tile box of the three stencil sources Y_u, A_u, B_u
+  CUtensorMap tm_box[10];
+  CUtensorMap tm_tile[3];
   std::vector<hr_puncture> punctures;
   HrGrid g;
   HrArrays a;
@@ -135,7 +149,7 @@ cudaError_t hrk_unpack(const hr_solver* s, void* dst_stored, const void* src_pub
 void hrk_row_geometry(int T0, int ng, size_t scalar_bytes, int* P0, int* off0);
 // residual partial sums + final deterministic pass into out2_dev
 cudaError_t hrk_residual(const hr_solver* s, int mode, double* out2_dev);
-MarchPlan hrk_make_plan(const int32_t n[3], int ng, int coord);
+MarchPlan hrk_make_plan(const int32_t n[3], int ng, int coord, int dtype);
 // shared-memory opt-in and persistent grid sizes of the marching kernels; before graph capture
 cudaError_t hrk_prepare(hr_solver* s);
 int hrk_max_partials(const int32_t n[3], int ng);

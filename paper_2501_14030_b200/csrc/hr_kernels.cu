@@ -21,10 +21,26 @@ namespace {
 // arithmetic shared by the RHS and the residual
 // ------------------------------------------------------------------------------------------
 
+// 1/x for x = psi_BL + u, which is >= 1 - |u| and of order one (psi_BL > 1, C1): the hardware
+// seed refined by Newton steps to full precision, without the denormal / overflow slow path a
+// general division carries (two branches and a call per point).
+__device__ __forceinline__ float rcp_near_one(float x) {
+  float r;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return fmaf(r, fmaf(-x, r, 1.0f), r);
+}
+__device__ __forceinline__ double rcp_near_one(double x) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));  // ~20 good bits
+  r = fma(r, fma(-x, r, 1.0), r);
+  r = fma(r, fma(-x, r, 1.0), r);
+  return fma(r, fma(-x, r, 1.0), r);
+}
+
 // (psi_BL + u)^-7 of Eq. 4/5: one reciprocal and four multiplies.
 template <typename T>
 __device__ __forceinline__ T pow_m7(T x) {
-  const T t = T(1) / x;
+  const T t = rcp_near_one(x);
   const T t2 = t * t;
   const T t4 = t2 * t2;
   return t4 * t2 * t;
@@ -55,29 +71,44 @@ struct StepArgs {
 //   4: Y   = ACC + dt/6 k
 // (yu, yv) = Y and (au, av) = ACC at this point, loaded by the caller where the stage needs them;
 // (wu, wv) returns what was stored to out (the value the point's ghost images take, C15).
+// Arithmetic of one stage: (wu, wv) = what the stage stores to out, (nu, nv) = the new running
+// sum ACC (stages 1-3).
 template <typename T, int STAGE>
-__device__ __forceinline__ void rk_combine_regs(const StepArgs<T>& a, int64_t c, T ku, T kv, T in_u,
-                                                T in_v, T yu, T yv, T au, T av, T& wu, T& wv) {
+__device__ __forceinline__ void rk_values(T dt, T ku, T kv, T in_u, T in_v, T yu, T yv, T au, T av,
+                                          T& wu, T& wv, T& nu, T& nv) {
+  nu = T(0);
+  nv = T(0);
   if constexpr (STAGE == 0) {
     wu = ku;
     wv = kv;
   } else if constexpr (STAGE == 1) {
-    const T h = a.dt * T(0.5), s = a.dt / T(6);
+    const T h = dt * T(0.5), s = dt / T(6);
     wu = in_u + h * ku;
     wv = in_v + h * kv;
-    a.acc_u[c] = in_u + s * ku;
-    a.acc_v[c] = in_v + s * kv;
+    nu = in_u + s * ku;
+    nv = in_v + s * kv;
   } else if constexpr (STAGE == 2 || STAGE == 3) {
-    const T h = (STAGE == 2) ? a.dt * T(0.5) : a.dt;
-    const T s = a.dt / T(3);
+    const T h = (STAGE == 2) ? dt * T(0.5) : dt;
+    const T s = dt / T(3);
     wu = yu + h * ku;
     wv = yv + h * kv;
-    a.acc_u[c] = au + s * ku;
-    a.acc_v[c] = av + s * kv;
+    nu = au + s * ku;
+    nv = av + s * kv;
   } else {
-    const T s = a.dt / T(6);
+    const T s = dt / T(6);
     wu = au + s * ku;
     wv = av + s * kv;
+  }
+}
+
+template <typename T, int STAGE>
+__device__ __forceinline__ void rk_combine_regs(const StepArgs<T>& a, int64_t c, T ku, T kv, T in_u,
+                                                T in_v, T yu, T yv, T au, T av, T& wu, T& wv) {
+  T nu, nv;
+  rk_values<T, STAGE>(a.dt, ku, kv, in_u, in_v, yu, yv, au, av, wu, wv, nu, nv);
+  if constexpr (STAGE >= 1 && STAGE <= 3) {
+    a.acc_u[c] = nu;
+    a.acc_v[c] = nv;
   }
   a.out_u[c] = wu;
   a.out_v[c] = wv;
@@ -383,39 +414,124 @@ cudaError_t launch_substep_direct(const hr_solver* s, int stage, void* ku, void*
 }
 
 // ---- marching arrangement (variant 0) ----
+// Tile shape per dtype: TW x BY points, VX points per thread (16-byte vectors along i0 are
+// double2 / float4; fp64 keeps one point per thread for register room), D planes of look-ahead.
 template <typename T>
-constexpr int march_depth() {
-  return sizeof(T) == 8 ? HR_MARCH_D_F64 : HR_MARCH_D_F32;
+struct MarchCfg;
+template <>
+struct MarchCfg<double> {
+  static constexpr int TW = HR_TW_F64, BY = HR_BY_F64, VX = HR_VX_F64, D = HR_MARCH_D_F64;
+};
+template <>
+struct MarchCfg<float> {
+  static constexpr int TW = HR_TW_F32, BY = HR_BY_F32, VX = HR_VX_F32, D = HR_MARCH_D_F32;
+};
+
+#define HR_MARCH_KERNEL(T, NG, STAGE) \
+  k_march<T, NG, STAGE, MarchCfg<T>::TW, MarchCfg<T>::BY, MarchCfg<T>::VX, MarchCfg<T>::D>
+#define HR_MARCH_SMEM(T, NG, STAGE) \
+  march_smem_bytes<T, NG, STAGE, MarchCfg<T>::TW, MarchCfg<T>::BY, MarchCfg<T>::D>()
+
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda).
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*,
+                                  const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+cudaError_t encode_box(const hr_solver* s, CUtensorMap* map, void* base, int bw, int bh) {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q);
+    if (e != cudaSuccess) return e;
+    if (!p || q != cudaDriverEntryPointSuccess) return cudaErrorNotSupported;
+    fn = reinterpret_cast<EncodeTiledFn>(p);
+  }
+  const HrGrid& g = s->g;
+  const cuuint64_t w = s->scalar_bytes;
+  const cuuint64_t dims[3] = {(cuuint64_t)g.P0, (cuuint64_t)g.T1, (cuuint64_t)g.T2};
+  const cuuint64_t strides[2] = {(cuuint64_t)g.P0 * w, (cuuint64_t)g.P0 * g.T1 * w};
+  const cuuint32_t box[3] = {(cuuint32_t)bw, (cuuint32_t)bh, 1u};
+  const cuuint32_t estr[3] = {1u, 1u, 1u};
+  const CUresult r = fn(map, w == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32,
+                        3, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                        CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+
+// Planes per chunk: work items = tiles x chunks are dealt round-robin to `slots` persistent CTAs,
+// so the last round is only partly full.  Among chunk counts that keep a chunk at least
+// max(2NG, 6) planes long (each item primes a 2NG-plane window) pick the one that wastes the
+// least of the last round; ties go to the longer chunk.
+static void choose_chunks(MarchPlan& m, int n2, int ng, int slots) {
+  const char* zc_env = std::getenv("HR_TUNE_ZC");  // tuning knob: planes per chunk
+  if (zc_env && std::atoi(zc_env) > 0) {
+    m.zc = std::atoi(zc_env) < n2 ? std::atoi(zc_env) : n2;
+    m.nzc = (n2 + m.zc - 1) / m.zc;
+    return;
+  }
+  const int ntiles = m.ntx * m.nty;
+  const int min_zc = 2 * ng > 6 ? 2 * ng : 6;
+  int best_nzc = 1;
+  double best = -1.0;
+  for (int nzc = 1; nzc <= n2; ++nzc) {
+    const int zc = (n2 + nzc - 1) / nzc;
+    if (nzc > 1 && zc < min_zc) break;
+    if ((n2 + zc - 1) / zc != nzc) continue;  // not a distinct chunking
+    const long long items = (long long)ntiles * nzc;
+    const long long rounds = (items + slots - 1) / slots;
+    // time ~ rounds x (zc + priming); useful work ~ items x zc / slots
+    const double eff = ((double)items * zc / slots) / ((double)rounds * (zc + 0.25 * ng + 1.0));
+    if (eff > best + 1e-9) {
+      best = eff;
+      best_nzc = nzc;
+    }
+  }
+  m.nzc = best_nzc;
+  m.zc = (n2 + best_nzc - 1) / best_nzc;
 }
 
 // Persistent grid of one stage's kernel: resident CTAs per SM x SMs (never more than the work).
 template <typename T, int NG, int STAGE>
 cudaError_t prepare_march_stage(const hr_solver* s, int* grid_out) {
-  constexpr int D = march_depth<T>();
-  auto kern = k_march<T, NG, STAGE, HR_TILE_BX, HR_TILE_BY, D>;
-  constexpr size_t smem = march_smem_bytes<T, NG, STAGE, HR_TILE_BX, HR_TILE_BY, D>();
+  using C = MarchCfg<T>;
+  auto kern = HR_MARCH_KERNEL(T, NG, STAGE);
+  constexpr size_t smem = HR_MARCH_SMEM(T, NG, STAGE);
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   int per_sm = 0;
-  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, HR_TILE_BX * HR_TILE_BY, smem);
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, (C::TW / C::VX) * C::BY, smem);
   if (e != cudaSuccess) return e;
   if (per_sm < 1) return cudaErrorLaunchOutOfResources;
-  const long long total = (long long)s->plan.ntx * s->plan.nty * s->plan.nzc;
-  long long grid = (long long)per_sm * s->num_sms;
-  if (grid > total) grid = total;
-  *grid_out = (int)grid;
+  *grid_out = per_sm * s->num_sms;
   return cudaSuccess;
 }
 
 template <typename T, int NG>
 cudaError_t prepare_march(hr_solver* s) {
+  using C = MarchCfg<T>;
+  using G = MarchGeom<T, NG, C::TW, C::BY>;
   cudaError_t e;
+  const HrArrays& a = s->a;
+  void* fields[10] = {a.Y[0], a.Y[1], a.A[0], a.A[1], a.B[0], a.B[1], a.ACC[0], a.ACC[1], a.psi, a.S};
+  for (int f = 0; f < 10; ++f)
+    if ((e = encode_box(s, &s->tm_box[f], fields[f], C::TW, C::BY)) != cudaSuccess) return e;
+  for (int f = 0; f < 3; ++f)
+    if ((e = encode_box(s, &s->tm_tile[f], fields[2 * f], G::SWA, G::SH)) != cudaSuccess) return e;
   if ((e = prepare_march_stage<T, NG, 0>(s, &s->march_grid[0])) != cudaSuccess) return e;
   if ((e = prepare_march_stage<T, NG, 1>(s, &s->march_grid[1])) != cudaSuccess) return e;
   if ((e = prepare_march_stage<T, NG, 2>(s, &s->march_grid[2])) != cudaSuccess) return e;
   if ((e = prepare_march_stage<T, NG, 3>(s, &s->march_grid[3])) != cudaSuccess) return e;
   if ((e = prepare_march_stage<T, NG, 4>(s, &s->march_grid[4])) != cudaSuccess) return e;
-  return prepare_march_stage<T, NG, 5>(s, &s->march_grid[5]);
+  if ((e = prepare_march_stage<T, NG, 5>(s, &s->march_grid[5])) != cudaSuccess) return e;
+  // one chunking for all stages, balanced for the RK stage kernels (stages 2, 3 dominate)
+  choose_chunks(s->plan, s->g.n2, NG, s->march_grid[2]);
+  const long long items = (long long)s->plan.ntx * s->plan.nty * s->plan.nzc;
+  for (int st = 0; st < 6; ++st)
+    if (s->march_grid[st] > items) s->march_grid[st] = (int)items;
+  return cudaSuccess;
 }
 
 template <typename T>
@@ -431,13 +547,30 @@ cudaError_t prepare_march_ng(hr_solver* s) {
   return cudaErrorInvalidValue;
 }
 
+// Tensor maps of one stage: stencil source = Y (stages 0, 1, residual), A (2, 4), B (3).
+MarchMaps make_maps(const hr_solver* s, int stage) {
+  const int in = (stage == 2 || stage == 4) ? 1 : (stage == 3 ? 2 : 0);
+  MarchMaps m;
+  m.tile = s->tm_tile[in];
+  m.st[ST_FRONT] = s->tm_box[2 * in];
+  m.st[ST_V] = s->tm_box[2 * in + 1];
+  m.st[ST_PSI] = s->tm_box[8];
+  m.st[ST_S] = s->tm_box[9];
+  m.st[ST_AU] = s->tm_box[6];
+  m.st[ST_AV] = s->tm_box[7];
+  m.st[ST_YU] = s->tm_box[0];
+  m.st[ST_YV] = s->tm_box[1];
+  return m;
+}
+
 template <typename T, int NG, int STAGE>
 cudaError_t launch_march_stage(const hr_solver* s, const StepArgs<T>& a, const ResidArgs& ra) {
-  constexpr int D = march_depth<T>();
-  constexpr size_t smem = march_smem_bytes<T, NG, STAGE, HR_TILE_BX, HR_TILE_BY, D>();
-  const dim3 block(HR_TILE_BX, HR_TILE_BY, 1);
+  using C = MarchCfg<T>;
+  constexpr size_t smem = HR_MARCH_SMEM(T, NG, STAGE);
+  const dim3 block(C::TW / C::VX, C::BY, 1);
   const dim3 grid(s->march_grid[STAGE], 1, 1);
-  k_march<T, NG, STAGE, HR_TILE_BX, HR_TILE_BY, D><<<grid, block, smem, s->stream>>>(s->g, a, s->plan, ra);
+  const MarchMaps mm = make_maps(s, STAGE);
+  HR_MARCH_KERNEL(T, NG, STAGE)<<<grid, block, smem, s->stream>>>(s->g, a, s->plan, ra, mm);
   return cudaGetLastError();
 }
 
@@ -529,17 +662,17 @@ cudaError_t dispatch_residual(const hr_solver* s, int mode, double* out2) {
 
 }  // namespace
 
-// Tiling of the marching kernels for a grid.
-MarchPlan hrk_make_plan(const int32_t n[3], int ng, int coord) {
+// Tiling of the marching kernels for a grid.  The chunk length is fixed later (hrk_prepare),
+// once the persistent grid size is known.
+MarchPlan hrk_make_plan(const int32_t n[3], int ng, int coord, int dtype) {
   MarchPlan m{};
-  m.ntx = (n[0] + HR_TILE_BX - 1) / HR_TILE_BX;
-  m.nty = (n[1] + HR_TILE_BY - 1) / HR_TILE_BY;
+  const int tw = dtype == HR_F64 ? MarchCfg<double>::TW : MarchCfg<float>::TW;
+  const int by = dtype == HR_F64 ? MarchCfg<double>::BY : MarchCfg<float>::BY;
+  m.ntx = (n[0] + tw - 1) / tw;
+  m.nty = (n[1] + by - 1) / by;
   m.sph = coord == HR_SINHSPHERICAL ? 1 : 0;
-  const char* zc = std::getenv("HR_TUNE_ZC");  // tuning knob: planes per chunk
-  m.zc = zc ? std::atoi(zc) : 16;
-  if (m.zc > n[2]) m.zc = n[2];
-  if (m.zc < 1) m.zc = 1;
-  m.nzc = (n[2] + m.zc - 1) / m.zc;
+  m.zc = n[2];
+  m.nzc = 1;
   (void)ng;
   return m;
 }

@@ -1,17 +1,20 @@
 // hr_march.cuh -- the default arrangement of the fused substep and of the residual on sm_100a:
-// 2.5-D blocking.  One CTA owns a BX x BY tile of (i0, i1) and marches along i2 over a chunk of
-// planes.
-//   * every global load of the loop is asynchronous (cp.async / LDGSTS into shared memory) and
-//     issued D planes ahead of its use, so no memory round trip sits on an iteration's critical
-//     path and the bytes in flight do not depend on occupancy: per plane a thread fetches its
-//     share of the (i0, i1) halo ring of the stage's u, the next value of its i2 pipeline, and
-//     its own pointwise inputs (v, psi_BL, S, Y, ACC) into private slots of a (D+1)-deep ring;
-//   * the tile centre is stored from registers one plane ahead; one __syncthreads per plane;
-//   * the i2 stencil is a register pipeline of 2 NG + 1 values per thread;
-//   * CTAs are persistent: the (tile, plane) iterations are split evenly over the resident CTAs,
-//     each CTA marching one or more column segments, so there is no wave-quantisation tail;
+// 2.5-D blocking with TMA.  One CTA owns a TW x BY tile of (i0, i1) and marches along i2.
+//   * every load of the loop is a TMA box copy (cp.async.bulk.tensor.3d) issued by one thread D
+//     planes ahead of its use into a (D+1)-deep shared-memory ring and completed on an mbarrier:
+//     per plane the (i0, i1) halo tile of the stage's u, the next plane of the i2 window, and the
+//     tile's pointwise inputs (v, psi_BL, S, Y, ACC).  No memory round trip sits on an
+//     iteration's critical path, the bytes in flight do not depend on occupancy, and the
+//     compute threads spend no instructions on load addresses;
+//   * a thread owns VX consecutive points along i0 and reads / writes them as one vector
+//     (rows of the stored layout start on 128-byte lines, hr_internal.h);
+//   * the i2 stencil is a register window of 2 NG + 1 planes per point; the plane loop is
+//     unrolled 2 NG + 1 times so the window rotates through the registers without moves;
+//   * CTAs are persistent over (chunk of planes, tile) work items in chunk-major order, so the
+//     CTAs resident at any time work on neighbouring tiles of the same planes (halo rows meet
+//     in L2);
 //   * the reference-metric factors depend on (i0, i1) only (reading C4), so each thread loads its
-//     six coefficients once and keeps them in registers for the whole column;
+//     six coefficients once per column and keeps them in registers;
 //   * the RK combine (a4) happens in the same thread, so k never reaches HBM, and the thread that
 //     produces a point also writes that point's inner-ghost images (a3, reading C14/C15) --
 //     closed-form integer arithmetic, the inverse of the host's inner map -- so a substep is
@@ -26,45 +29,81 @@ struct ResidArgs {
   int mode;
 };
 
-__device__ __forceinline__ void cp_async_scalar(double* smem_dst, const double* gsrc) {
-  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(d), "l"(gsrc) : "memory");
+template <typename T, int VX>
+struct alignas(sizeof(T) * VX) Vec {
+  T v[VX];
+};
+
+// Tensor maps of one launch: the halo-tile box of the stage's u and the TW x BY box of every
+// pointwise input, indexed by ST_*.
+struct alignas(64) MarchMaps {
+  CUtensorMap tile;
+  CUtensorMap st[8];
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+  return (uint32_t)__cvta_generic_to_shared(p);
 }
-__device__ __forceinline__ void cp_async_scalar(float* smem_dst, const float* gsrc) {
-  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;\n" ::"r"(d), "l"(gsrc) : "memory");
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count) : "memory");
 }
-__device__ __forceinline__ void prefetch_l2(const void* p) {
-  asm volatile("prefetch.global.L2 [%0];\n" ::"l"(p));
+__device__ __forceinline__ void mbar_fence_init() {
+  asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+  asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
 }
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait_group() {
-  asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory");
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)),
+               "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t phase) {
+  uint32_t ok;
+  uint32_t spins = 0;
+  do {
+    if (++spins > (1u << 24)) __trap();  // a lost TMA transaction must fail loudly, not hang
+    asm volatile(
+        "{\n.reg .pred p;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n}\n"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(phase)
+        : "memory");
+  } while (!ok);
+}
+__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, int x, int y, int z,
+                                            uint64_t* bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes "
+      "[%0], [%1, {%2, %3, %4}], [%5];\n" ::"r"(smem_u32(dst)),
+      "l"(map), "r"(x), "r"(y), "r"(z), "r"(smem_u32(bar))
+      : "memory");
 }
 
 // Inner-ghost images of the point (j0, j1, j2) that was just written (j0 >= NG, j1 and j2
 // interior): every ghost point whose source under the host's inner map (hr_api.cu:
 // inner_source, reading C14) is this point.  r0 = 2NG-1-j0 if j0 < 2NG else -1; cB / cC = the
 // theta-low / theta-high reflections of j1 or -1.  Each flip shifts phi by pi; phi is periodic.
+// Not inlined: few points have images, and the plane loop is unrolled 2NG+1 times -- inlining
+// this per point and per copy pushed the stage kernels out of the instruction cache.
+struct ImgGeom {
+  int ng, n2, T1, P0, off0, sph;
+};
 template <typename T>
-__device__ __forceinline__ void scatter_images(const HrGrid& g, int sph, T* __restrict__ ou,
-                                               T* __restrict__ ov, T vu, T vv, int j0, int j1,
-                                               int j2, int r0, int cB, int cC) {
+__device__ __noinline__ void scatter_images(ImgGeom g, T* __restrict__ ou, T* __restrict__ ov, T vu,
+                                            T vv, int j0, int j1, int j2, int r0, int cB, int cC) {
   const int ng = g.ng;
   const int kbase = j2 - ng;
   const int half = g.n2 >> 1;
   const int s2 = g.P0 * g.T1;
-#pragma unroll
+#pragma unroll 1
   for (int f0 = 0; f0 < 2; ++f0) {
     if (f0 && r0 < 0) continue;
     const int d0 = f0 ? r0 : j0;
-#pragma unroll
+#pragma unroll 1
     for (int m = 0; m < 3; ++m) {
       const int c = m == 0 ? j1 : (m == 1 ? cB : cC);
       if (c < 0) continue;
-      const int d1 = (f0 && sph) ? g.T1 - 1 - c : c;
+      const int d1 = (f0 && g.sph) ? g.T1 - 1 - c : c;
       const int flips = f0 + (m != 0);
       int kd = kbase - ((flips & 1) ? half : 0);
       if (kd < 0) kd += g.n2;
@@ -88,8 +127,75 @@ __device__ __forceinline__ void scatter_images(const HrGrid& g, int sph, T* __re
   }
 }
 
+// The same for the VX points (i0 .. i0+VX-1, i1, z) a marching thread has just written, with the
+// common cases first: the phi-periodic images of the points themselves and the theta-reflected
+// rows are whole-vector stores; only the rho -> -rho reflections (first 2NG points of a row) go
+// point by point.  Not inlined (see above); called for boundary planes / boundary threads only.
+template <typename T, int VX>
+__device__ __noinline__ void scatter_vec(ImgGeom g, T* __restrict__ ou, T* __restrict__ ov,
+                                         Vec<T, VX> wu, Vec<T, VX> wv, int i0, int i1, int z,
+                                         int nact, int cB, int cC) {
+  const int ng = g.ng, n2 = g.n2;
+  const int s2 = g.P0 * g.T1;
+  const int k0 = z - ng;  // phi index of the source
+  int k1 = k0 - (n2 >> 1);  // after an odd number of flips
+  if (k1 < 0) k1 += n2;
+  auto store_v = [&](int d) {
+    if (nact == VX) {
+      *reinterpret_cast<Vec<T, VX>*>(ou + d) = wu;
+      *reinterpret_cast<Vec<T, VX>*>(ov + d) = wv;
+    } else {
+#pragma unroll
+      for (int j = 0; j < VX; ++j)
+        if (j < nact) {
+          ou[d + j] = wu.v[j];
+          ov[d + j] = wv.v[j];
+        }
+    }
+  };
+  auto put_v = [&](int rowbase, int k, bool main) {
+    if (main) store_v(rowbase + (k + ng) * s2);
+    if (k < ng) store_v(rowbase + (k + ng + n2) * s2);
+    if (k >= n2 - ng) store_v(rowbase + (k + ng - n2) * s2);
+  };
+  const int rb = g.off0 + i0;
+  put_v(rb + g.P0 * i1, k0, false);
+  if (cB >= 0) put_v(rb + g.P0 * cB, k1, true);
+  if (cC >= 0) put_v(rb + g.P0 * cC, k1, true);
+  if (i0 < 2 * ng) {
+#pragma unroll
+    for (int j = 0; j < VX; ++j) {
+      if (j >= nact || i0 + j >= 2 * ng) continue;
+      const int rr = g.off0 + 2 * ng - 1 - (i0 + j);
+      const T vu = wu.v[j], vv = wv.v[j];
+#pragma unroll 1
+      for (int m = 0; m < 3; ++m) {
+        const int c = m == 0 ? i1 : (m == 1 ? cB : cC);
+        if (c < 0) continue;
+        const int d1 = g.sph ? g.T1 - 1 - c : c;
+        const int k = m == 0 ? k1 : k0;  // one flip, or two
+        const int rowbase = rr + g.P0 * d1;
+        {
+          const int d = rowbase + (k + ng) * s2;
+          ou[d] = vu;
+          ov[d] = vv;
+        }
+        if (k < ng) {
+          const int d = rowbase + (k + ng + n2) * s2;
+          ou[d] = vu;
+          ov[d] = vv;
+        }
+        if (k >= n2 - ng) {
+          const int d = rowbase + (k + ng - n2) * s2;
+          ou[d] = vu;
+          ov[d] = vv;
+        }
+      }
+    }
+  }
+}
 
-// Slots of a thread's private stream ring, in the order the stages need them.
+// Boxes of a ring slot, in the order the stages need them.
 enum { ST_FRONT = 0, ST_PSI = 1, ST_S = 2, ST_V = 3, ST_AU = 4, ST_AV = 5, ST_YU = 6, ST_YV = 7 };
 
 template <int STAGE>
@@ -97,42 +203,73 @@ __host__ __device__ constexpr int march_nstreams() {
   return STAGE == 5 ? 3 : (STAGE <= 1 ? 4 : (STAGE == 4 ? 6 : 8));
 }
 
-template <typename T, int NG, int STAGE, int BX, int BY, int D>
+// Geometry shared by the kernel and the host (tensor-map boxes, shared-memory size).
+//   NGA  halo width of the tile along i0, NG rounded up so that box rows are whole 16-byte units
+//   SWA  tile row length, SH tile rows
+template <typename T, int NG, int TW, int BY>
+struct MarchGeom {
+  static constexpr int Q = 16 / (int)sizeof(T);
+  static constexpr int NGA = (NG + Q - 1) / Q * Q;
+  static constexpr int SWA = TW + 2 * NGA;
+  static constexpr int SH = BY + 2 * NG;
+  static constexpr int TILE_BYTES = (SWA * SH * (int)sizeof(T) + 127) / 128 * 128;
+  static constexpr int BOX_BYTES = TW * BY * (int)sizeof(T);
+  static_assert(BOX_BYTES % 128 == 0, "stream boxes must keep 128-byte alignment");
+};
+
+template <typename T, int NG, int STAGE, int TW, int BY, int D>
 __host__ __device__ constexpr size_t march_smem_bytes() {
-  return sizeof(T) * (size_t)(D + 1) *
-         ((size_t)(BX + 2 * NG) * (BY + 2 * NG) + (size_t)march_nstreams<STAGE>() * BX * BY);
+  using G = MarchGeom<T, NG, TW, BY>;
+  return 128 + (size_t)(D + 1) * (G::TILE_BYTES + march_nstreams<STAGE>() * G::BOX_BYTES);
 }
 
 // STAGE 0: k -> out (hr_eval_rhs); 1..4: RK4 stages (rk_combine); 5: residual (a5).
-// D = planes of asynchronous look-ahead.
-template <typename T, int NG, int STAGE, int BX, int BY, int D>
-__global__ void __launch_bounds__(BX* BY, sizeof(T) == 8 ? HR_MARCH_MINB_F64 : HR_MARCH_MINB_F32)
+// TW x BY points per tile, VX points per thread along i0, D planes of look-ahead.
+template <typename T, int NG, int STAGE, int TW, int BY, int VX, int D>
+__global__ void __launch_bounds__((TW / VX) * BY,
+                                  sizeof(T) == 8 ? HR_MARCH_MINB_F64 : HR_MARCH_MINB_F32)
     k_march(const __grid_constant__ HrGrid g, const __grid_constant__ StepArgs<T> a,
-            const __grid_constant__ MarchPlan plan, const __grid_constant__ ResidArgs ra) {
-  constexpr int NT = BX * BY;
-  constexpr int SW = BX + 2 * NG, SH = BY + 2 * NG;
-  constexpr int TILE = SW * SH;
-  constexpr int NHALO = TILE - NT;
-  constexpr int NSLOT = (NHALO + NT - 1) / NT;
+            const __grid_constant__ MarchPlan plan, const __grid_constant__ ResidArgs ra,
+            const __grid_constant__ MarchMaps mm) {
+  using G = MarchGeom<T, NG, TW, BY>;
+  using V = Vec<T, VX>;
+  using F = FdTable<NG>;
+  constexpr int BXT = TW / VX;  // threads along i0
+  constexpr int NT = BXT * BY;
+  constexpr int NGA = G::NGA, SWA = G::SWA;
+  constexpr int NGV = (NG + VX - 1) / VX * VX;  // halo rounded to whole vectors
   constexpr int NS = march_nstreams<STAGE>();
   constexpr int RING = D + 1;
-  using F = FdTable<NG>;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  T* const tiles = reinterpret_cast<T*>(smem_raw);  // [RING][SH][SW]
-  T* const strm = tiles + RING * TILE;              // [RING][NS][NT]
+  constexpr int SLOT_BYTES = G::TILE_BYTES + NS * G::BOX_BYTES;
+  constexpr int U = 2 * NG + 1;
+  // UR = U: the plane loop is unrolled U times and the i2 window rotates through the registers
+  // without moves; UR = 1: one copy of the body (fits the 32 KB instruction cache) and the
+  // window is shifted with register moves.
+  constexpr int UR = HR_MARCH_ROTATE ? U : 1;
+  static_assert(NGA % VX == 0 && TW % VX == 0, "vector alignment");
+
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  uint64_t* const bars = reinterpret_cast<uint64_t*>(smem_raw);  // [RING] "slot is full"
+  unsigned char* const ring = smem_raw + 128;
 
   const int lx = threadIdx.x, ly = threadIdx.y;
-  const int tid = ly * BX + lx;
+  const int tid = ly * BXT + lx;
   const int s2 = g.P0 * g.T1;
-  const T* __restrict__ uin = a.in_u;
-  const int ctr = (ly + NG) * SW + lx + NG;  // this thread's point in a tile
+  const ImgGeom ig{NG, g.n2, g.T1, g.P0, g.off0, plan.sph};
 
-  // work items = (chunk of planes, tile), chunk-major, so that the CTAs resident at any time work
-  // on neighbouring tiles of the same planes (halo rows and partial lines meet in L2)
+  if (tid == 0) {
+#pragma unroll
+    for (int r = 0; r < RING; ++r) mbar_init(&bars[r], 1);
+    mbar_fence_init();
+  }
+  __syncthreads();
+
+  // work items = (chunk of planes, tile), chunk-major
   const int ntiles = plan.ntx * plan.nty;
   const int n_items = ntiles * plan.nzc;
 
   double num = 0.0, den = 0.0;
+  unsigned n_cons = 0;  // planes consumed so far by this CTA: slot = n % RING, parity = n / RING
 
   for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
     const int chunk = item / ntiles;
@@ -141,155 +278,190 @@ __global__ void __launch_bounds__(BX* BY, sizeof(T) == 8 ? HR_MARCH_MINB_F64 : H
     const int seg = min(plan.zc, g.n2 - zi);
     const int tx = tile_id % plan.ntx, ty = tile_id / plan.ntx;
     const int z_begin = NG + zi, z_end = z_begin + seg;
-    const int i0 = NG + tx * BX + lx, i1 = NG + ty * BY + ly;
-    const bool active = i0 < g.n0 + NG && i1 < g.n1 + NG;
-    // inactive threads of edge tiles still feed the tile centre (their points are ghosts that
-    // the neighbours' stencils read), so they track real grid values, clamped to the grid
-    const int col = g.off0 + min(i0, g.T0 - 1) + g.P0 * min(i1, g.T1 - 1);
+    const int x0 = NG + tx * TW, y0 = NG + ty * BY;  // first point of the tile
+    const int i0 = x0 + VX * lx, i1 = y0 + ly;
+    // number of this thread's points that are interior (0..VX)
+    const int nact = i1 < g.n1 + NG ? max(0, min(VX, g.n0 + NG - i0)) : 0;
+    const int col = g.off0 + i0 + g.P0 * i1;  // only dereferenced if nact > 0
 
-    // halo ring slots of this thread: tile offset and in-plane global offset (-1: none)
-    int h_s[NSLOT], h_g[NSLOT];
+    // one thread feeds the ring: everything plane zz needs, into slot (n_cons + d) % RING
+    auto issue = [&](int zz, unsigned n) {
+      const unsigned sl = n % RING;
+      unsigned char* base = ring + sl * SLOT_BYTES;
+      uint64_t* bar = &bars[sl];
+      mbar_expect_tx(bar, (uint32_t)(SWA * G::SH * sizeof(T) + NS * G::BOX_BYTES));
+      const int xs = g.off0 + x0;
+      tma_load_3d(base, &mm.tile, xs - NGA, y0 - NG, zz, bar);
+      unsigned char* sb = base + G::TILE_BYTES;
+      tma_load_3d(sb + ST_FRONT * G::BOX_BYTES, &mm.st[ST_FRONT], xs, y0, zz + NG, bar);
 #pragma unroll
-    for (int s = 0; s < NSLOT; ++s) {
-      const int h = tid + s * NT;
-      int r, c;
-      if (h < 2 * NG * SW) {
-        r = h / SW;
-        c = h - r * SW;
-        if (r >= NG) r += BY;
-      } else {
-        const int hh = h - 2 * NG * SW;
-        r = NG + hh / (2 * NG);
-        c = hh % (2 * NG);
-        if (c >= NG) c += BX;
-      }
-      const int gi0 = tx * BX + c, gi1 = ty * BY + r;
-      h_s[s] = r * SW + c;
-      h_g[s] = (h < NHALO && gi0 < g.T0 && gi1 < g.T1) ? g.off0 + gi0 + g.P0 * gi1 : -1;
+      for (int q = 1; q < NS; ++q) tma_load_3d(sb + q * G::BOX_BYTES, &mm.st[q], xs, y0, zz, bar);
+    };
+    if (tid == 0) {
+#pragma unroll
+      for (int d = 0; d < D; ++d)
+        if (z_begin + d < z_end) issue(z_begin + d, n_cons + d);
     }
 
     // per-column constants
-    T l00 = T(0), l11 = T(0), l22 = T(0), l0 = T(0), l1 = T(0), c2 = T(0);
-    double wq = 0.0;
-    int r0 = -1, cB = -1, cC = -1;
-    if (active) {
-      const int q = i0 + g.T0 * i1;
-      l00 = a.L00[q]; l11 = a.L11[q]; l22 = a.L22[q]; l0 = a.L0[q]; l1 = a.L1[q];
-      if constexpr (STAGE == 5) {
-        wq = ra.mode == 0 ? ra.W[q] : 1.0;
-      } else {
-        c2 = a.C2[q];
-        r0 = i0 < 2 * NG ? 2 * NG - 1 - i0 : -1;
-        cB = i1 < 2 * NG ? 2 * NG - 1 - i1 : -1;
-        cC = i1 >= g.n1 ? 2 * (g.n1 + NG) - 1 - i1 : -1;
+    T l00[VX], l11[VX], l22[VX], l0[VX], l1[VX], c2[VX];
+    double wq[VX];
+    int cB = -1, cC = -1;
+    bool inplane_images = false;
+#pragma unroll
+    for (int j = 0; j < VX; ++j) {
+      l00[j] = l11[j] = l22[j] = l0[j] = l1[j] = c2[j] = T(0);
+      wq[j] = 0.0;
+      if (j < nact) {
+        const int q = i0 + j + g.T0 * i1;
+        l00[j] = a.L00[q]; l11[j] = a.L11[q]; l22[j] = a.L22[q]; l0[j] = a.L0[q]; l1[j] = a.L1[q];
+        if constexpr (STAGE == 5) {
+          wq[j] = ra.mode == 0 ? ra.W[q] : 1.0;
+        } else {
+          c2[j] = a.C2[q];
+          inplane_images |= i0 + j < 2 * NG;
+        }
       }
     }
-    const bool inplane_images = (r0 >= 0) || (cB >= 0) || (cC >= 0);
+    if (STAGE != 5 && nact > 0) {
+      cB = i1 < 2 * NG ? 2 * NG - 1 - i1 : -1;
+      cC = i1 >= g.n1 ? 2 * (g.n1 + NG) - 1 - i1 : -1;
+      inplane_images |= (cB >= 0) || (cC >= 0);
+    }
 
-    // everything plane zz needs from global memory, as one cp.async group into ring slot sl
-    auto issue = [&](int zz, int sl) {
-      if (zz < z_end) {
-        T* tl = tiles + sl * TILE;
-        T* st = strm + sl * (NS * NT) + tid;
-        const int pl = zz * s2;
+    // register window: w(k)[j] = u(i0 + j, i1, z - NG + k), k = 0..2NG, kept in p[(r + k) % U]
+    // with r = (z - z_begin) % U (the plane loop is unrolled U times)
+    T p[U][VX];
+    if (nact > 0) {
 #pragma unroll
-        for (int s = 0; s < NSLOT; ++s)
-          if (h_g[s] >= 0) cp_async_scalar(tl + h_s[s], uin + h_g[s] + pl);
-        const int c = col + pl;
-        cp_async_scalar(st + ST_FRONT * NT, uin + c + NG * s2);
-        if (active) {
-          cp_async_scalar(st + ST_PSI * NT, a.psi + c);
-          cp_async_scalar(st + ST_S * NT, a.S + c);
-          if constexpr (STAGE != 5) cp_async_scalar(st + ST_V * NT, a.in_v + c);
-          if constexpr (STAGE >= 2 && STAGE <= 4) {
-            cp_async_scalar(st + ST_AU * NT, a.acc_u + c);
-            cp_async_scalar(st + ST_AV * NT, a.acc_v + c);
-          }
-          if constexpr (STAGE == 2 || STAGE == 3) {
-            cp_async_scalar(st + ST_YU * NT, a.y_u + c);
-            cp_async_scalar(st + ST_YV * NT, a.y_v + c);
-          }
-        }
+      for (int k = 0; k < 2 * NG; ++k) {
+        const V t = *reinterpret_cast<const V*>(a.in_u + col + (z_begin - NG + k) * s2);
+#pragma unroll
+        for (int j = 0; j < VX; ++j) p[k + (UR == 1 ? 1 : 0)][j] = t.v[j];
       }
-      cp_async_commit();
-    };
+    }
 
-    // prologue: look-ahead groups, then the register pipeline.  w(k) = u(i0, i1, z - NG + k),
-    // k = 0..2NG, lives in p[(j + k) % U] where j = (z - z_begin) % U: the plane loop is unrolled
-    // U = 2NG+1 times so the window rotates through the registers without moves.
+    const int so = ly * TW + VX * lx;                                     // in a TW x BY box
+    const int to = (ly + NG) * SWA + NGA + VX * lx;                       // in the halo tile
+    constexpr int NE = 2 * NGV + VX;                                      // row values a thread reads
+    for (int zb = z_begin; zb < z_end; zb += UR) {
 #pragma unroll
-    for (int d = 0; d < D; ++d) issue(z_begin + d, d);
-    constexpr int U = 2 * NG + 1;
-    T p[U];
-#pragma unroll
-    for (int k = 0; k < 2 * NG; ++k) p[k] = uin[col + (z_begin - NG + k) * s2];
-    tiles[ctr] = p[NG];
-
-    int sl = 0;  // ring slot of plane z
-    for (int zb = z_begin; zb < z_end; zb += U) {
-#pragma unroll
-      for (int j = 0; j < U; ++j) {
-        const int z = zb + j;
+      for (int r = 0; r < UR; ++r) {
+        const int z = zb + r;
         if (z >= z_end) break;
-#define HR_W(k) p[(j + (k)) % U]
-        cp_async_wait_group<D - 1>();  // this thread's group of plane z has landed
-        __syncthreads();               // everyone's has; slot of plane z-1 is free again
-        {
-          int sn = sl + D;
-          if (sn >= RING) sn -= RING;
-          issue(z + D, sn);
-        }
-        const T* tl = tiles + sl * TILE;
-        const T* st = strm + sl * (NS * NT) + tid;
-        HR_W(2 * NG) = st[ST_FRONT * NT];
-        int sn1 = sl + 1;
-        if (sn1 >= RING) sn1 = 0;
-        if (z + 1 < z_end) tiles[sn1 * TILE + ctr] = HR_W(NG + 1);
-
-        if (active) {
-          const int c = col + z * s2;
-          const T uc = HR_W(NG);
-          T d00 = T(F::d2(0)) * uc, d11 = d00, d22 = d00, d0 = T(0), d1 = T(0);
+#define HR_W(k) p[(r + (k)) % U]
+        const unsigned sl = n_cons % RING;
+        __syncthreads();  // every thread is done with plane z-1: its slot can be refilled
+        if (tid == 0 && z + D < z_end) issue(z + D, n_cons + D);
+        mbar_wait(&bars[sl], (n_cons / RING) & 1u);  // the boxes of plane z have landed
+        ++n_cons;
+        if (nact > 0) {
+          if constexpr (UR == 1) {  // no rotation: shift the window by one plane
+#pragma unroll
+            for (int k = 0; k < 2 * NG; ++k)
+#pragma unroll
+              for (int j = 0; j < VX; ++j) p[k][j] = p[k + 1][j];
+          }
+          const T* tl = reinterpret_cast<const T*>(ring + sl * SLOT_BYTES);
+          const T* sb = reinterpret_cast<const T*>(ring + sl * SLOT_BYTES + G::TILE_BYTES);
+          {
+            const V fr = *reinterpret_cast<const V*>(sb + ST_FRONT * (TW * BY) + so);
+#pragma unroll
+            for (int j = 0; j < VX; ++j) HR_W(2 * NG)[j] = fr.v[j];
+          }
+          T e[NE];  // tile row of this thread: e[NGV + j + m] = u(i0 + j + m, i1, z)
+#pragma unroll
+          for (int m = 0; m < NE / VX; ++m) {
+            const V t = *reinterpret_cast<const V*>(tl + to - NGV + m * VX);
+#pragma unroll
+            for (int j = 0; j < VX; ++j) e[m * VX + j] = t.v[j];
+          }
+          T d00[VX], d11[VX], d22[VX], d0[VX], d1[VX];
+#pragma unroll
+          for (int j = 0; j < VX; ++j) {
+            d00[j] = T(F::d2(0)) * HR_W(NG)[j];
+            d11[j] = d00[j];
+            d22[j] = d00[j];
+            d0[j] = T(0);
+            d1[j] = T(0);
+          }
 #pragma unroll
           for (int k = 1; k <= NG; ++k) {
-            const T a0 = tl[ctr + k], b0 = tl[ctr - k];
-            const T a1 = tl[ctr + k * SW], b1 = tl[ctr - k * SW];
-            d00 += T(F::d2(k)) * (a0 + b0);
-            d11 += T(F::d2(k)) * (a1 + b1);
-            d22 += T(F::d2(k)) * (HR_W(NG + k) + HR_W(NG - k));
-            d0 += T(F::c1(k)) * (a0 - b0);
-            d1 += T(F::c1(k)) * (a1 - b1);
+            const V up = *reinterpret_cast<const V*>(tl + to + k * SWA);
+            const V dn = *reinterpret_cast<const V*>(tl + to - k * SWA);
+#pragma unroll
+            for (int j = 0; j < VX; ++j) {
+              const T a0 = e[NGV + j + k], b0 = e[NGV + j - k];
+              d00[j] += T(F::d2(k)) * (a0 + b0);
+              d11[j] += T(F::d2(k)) * (up.v[j] + dn.v[j]);
+              d22[j] += T(F::d2(k)) * (HR_W(NG + k)[j] + HR_W(NG - k)[j]);
+              d0[j] += T(F::c1(k)) * (a0 - b0);
+              d1[j] += T(F::c1(k)) * (up.v[j] - dn.v[j]);
+            }
           }
-          const T lap = l00 * d00 + l11 * d11 + l22 * d22 + l0 * d0 + l1 * d1;
-          const T H = lap + st[ST_S * NT] * pow_m7(st[ST_PSI * NT] + uc);
+          const V psi = *reinterpret_cast<const V*>(sb + ST_PSI * (TW * BY) + so);
+          const V Ss = *reinterpret_cast<const V*>(sb + ST_S * (TW * BY) + so);
+          T H[VX];
+#pragma unroll
+          for (int j = 0; j < VX; ++j) {
+            const T lap = l00[j] * d00[j] + l11[j] * d11[j] + l22[j] * d22[j] + l0[j] * d0[j] +
+                          l1[j] * d1[j];
+            H[j] = lap + Ss.v[j] * pow_m7(psi.v[j] + HR_W(NG)[j]);
+          }
           if constexpr (STAGE == 5) {
-            num += wq * (double)H * (double)H;
-            den += wq;
+#pragma unroll
+            for (int j = 0; j < VX; ++j)
+              if (j < nact) {
+                num += wq[j] * (double)H[j] * (double)H[j];
+                den += wq[j];
+              }
           } else {
-            const T vc = st[ST_V * NT];
-            T yu = T(0), yv = T(0), au = T(0), av = T(0);
+            const V vin = *reinterpret_cast<const V*>(sb + ST_V * (TW * BY) + so);
+            V yu{}, yv{}, au{}, av{};
             if constexpr (STAGE >= 2 && STAGE <= 4) {
-              au = st[ST_AU * NT];
-              av = st[ST_AV * NT];
+              au = *reinterpret_cast<const V*>(sb + ST_AU * (TW * BY) + so);
+              av = *reinterpret_cast<const V*>(sb + ST_AV * (TW * BY) + so);
             }
             if constexpr (STAGE == 2 || STAGE == 3) {
-              yu = st[ST_YU * NT];
-              yv = st[ST_YV * NT];
+              yu = *reinterpret_cast<const V*>(sb + ST_YU * (TW * BY) + so);
+              yv = *reinterpret_cast<const V*>(sb + ST_YV * (TW * BY) + so);
             }
-            const T ku = vc - a.eta * uc;
-            const T kv = c2 * H;
-            T wu, wv;
-            rk_combine_regs<T, STAGE>(a, c, ku, kv, uc, vc, yu, yv, au, av, wu, wv);
+            V wu, wv, nu, nv;  // stage output and the new running sum
+#pragma unroll
+            for (int j = 0; j < VX; ++j) {
+              const T uc = HR_W(NG)[j];
+              const T ku = vin.v[j] - a.eta * uc;
+              const T kv = c2[j] * H[j];
+              rk_values<T, STAGE>(a.dt, ku, kv, uc, vin.v[j], yu.v[j], yv.v[j], au.v[j], av.v[j],
+                                  wu.v[j], wv.v[j], nu.v[j], nv.v[j]);
+            }
+            const int c = col + z * s2;
+            if (nact == VX) {
+              *reinterpret_cast<V*>(a.out_u + c) = wu;
+              *reinterpret_cast<V*>(a.out_v + c) = wv;
+              if constexpr (STAGE >= 1 && STAGE <= 3) {
+                *reinterpret_cast<V*>(a.acc_u + c) = nu;
+                *reinterpret_cast<V*>(a.acc_v + c) = nv;
+              }
+            } else {
+#pragma unroll
+              for (int j = 0; j < VX; ++j)
+                if (j < nact) {
+                  a.out_u[c + j] = wu.v[j];
+                  a.out_v[c + j] = wv.v[j];
+                  if constexpr (STAGE >= 1 && STAGE <= 3) {
+                    a.acc_u[c + j] = nu.v[j];
+                    a.acc_v[c + j] = nv.v[j];
+                  }
+                }
+            }
             if (inplane_images || z < 2 * NG || z >= g.n2)
-              scatter_images<T>(g, plan.sph, a.out_u, a.out_v, wu, wv, i0, i1, z, r0, cB, cC);
+              scatter_vec<T, VX>(ig, a.out_u, a.out_v, wu, wv, i0, i1, z, nact, cB, cC);
           }
         }
-        if (++sl >= RING) sl = 0;
 #undef HR_W
       }
     }
-    cp_async_wait_all();
-    __syncthreads();  // the ring is reused by the next segment
   }
 
   if constexpr (STAGE == 5) {
@@ -333,7 +505,7 @@ __global__ void __launch_bounds__(BX* BY, sizeof(T) == 8 ? HR_MARCH_MINB_F64 : H
       const int cB = i1 < 2 * NG ? 2 * NG - 1 - i1 : -1;
       const int cC = i1 >= g.n1 ? 2 * (g.n1 + NG) - 1 - i1 : -1;
       if (cB >= 0 || cC >= 0 || i2 < 2 * NG || i2 >= g.n2)
-        scatter_images<T>(g, plan.sph, a.out_u, a.out_v, wu, wv, i0, i1, i2, -1, cB, cC);
+        scatter_images<T>(ig, a.out_u, a.out_v, wu, wv, i0, i1, i2, -1, cB, cC);
     }
   }
 }
