@@ -35,7 +35,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
     objs = []
     for src in SOURCES:
         obj = os.path.join(CSRC, src.replace(".cu", ".o"))
-        cmd = [_nvcc(), *NVCC_FLAGS, "-c", os.path.join(CSRC, src), "-o", obj]
+        # HR_NVCC_DEFS="-DHR_MARCH_D_F64=3 ...": tuning overrides of the macros in hr_internal.h
+        cmd = [_nvcc(), *NVCC_FLAGS, *os.environ.get("HR_NVCC_DEFS", "").split(), "-c",
+               os.path.join(CSRC, src), "-o", obj]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
         subprocess.run(cmd, check=True)

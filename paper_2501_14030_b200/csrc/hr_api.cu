@@ -82,7 +82,7 @@ struct Layout {
   size_t off_field[10];
   size_t off_plane[6];
   size_t off_rad[3];
-  size_t off_wvol, off_inner_dst, off_inner_src, off_partials, off_result;
+  size_t off_wvol, off_inner_dst, off_inner_src, off_partials, off_result, off_counters;
   size_t off_rho, off_rhoz, off_sinth, off_costh, off_sinph, off_cosph, off_punct;
   size_t total;
   int64_t ntot, n_inner, npad;
@@ -115,6 +115,7 @@ Layout make_layout(const hr_params* p) {
   L.nblocks = hrk_max_partials(p->n, L.ng);
   L.off_partials = take((size_t)L.nblocks * 16);
   L.off_result = take(64);
+  L.off_counters = take(256);
   L.off_rho = take((size_t)L.T[0] * 8);
   L.off_rhoz = take((size_t)L.T[0] * 8);
   L.off_sinth = take((size_t)L.T[1] * 8);
@@ -423,6 +424,8 @@ hr_status hr_create(const hr_params* p, void* workspace_dev, size_t workspace_by
   a.inner_src = reinterpret_cast<int32_t*>(base + L.off_inner_src);
   a.partials = reinterpret_cast<double*>(base + L.off_partials);
   a.result2 = reinterpret_cast<double*>(base + L.off_result);
+  s->plan.counters = reinterpret_cast<int*>(base + L.off_counters);
+  HR_CUDA(cudaMemsetAsync(s->plan.counters, 0, 256, s->stream));
   a.rho = reinterpret_cast<double*>(base + L.off_rho);
   a.rhoz = reinterpret_cast<double*>(base + L.off_rhoz);
   a.sinth = reinterpret_cast<double*>(base + L.off_sinth);

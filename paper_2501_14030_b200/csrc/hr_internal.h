@@ -86,7 +86,7 @@ struct HrArrays {
 
 // 1: unroll the plane loop 2NG+1 times (rotating register window); 0: single copy + moves.
 #ifndef HR_MARCH_ROTATE
-#define HR_MARCH_ROTATE 1
+#define HR_MARCH_ROTATE 0
 #endif
 
 // Planes of asynchronous look-ahead in the marching kernels.
@@ -101,6 +101,7 @@ struct HrArrays {
 struct MarchPlan {
   int ntx, nty;  // tiles along i0, i1
   int zc, nzc;   // planes per chunk, chunks along i2
+  int* counters; // device: {next item, CTAs done} per stage kernel, zero between launches
   int sph;       // 1 = SinhSpherical inner map (theta -> pi - theta under rho -> -rho)
 };
 

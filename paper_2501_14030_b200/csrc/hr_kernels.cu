@@ -461,10 +461,10 @@ cudaError_t encode_box(const hr_solver* s, CUtensorMap* map, void* base, int bw,
   return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
 
-// Planes per chunk: work items = tiles x chunks are dealt round-robin to `slots` persistent CTAs,
-// so the last round is only partly full.  Among chunk counts that keep a chunk at least
-// max(2NG, 6) planes long (each item primes a 2NG-plane window) pick the one that wastes the
-// least of the last round; ties go to the longer chunk.
+// Planes per chunk.  Work items = tiles x chunks are handed out dynamically to `slots` persistent
+// CTAs, so the run lasts about (all items' time) / slots plus one item of tail; an item costs its
+// planes plus about one plane of window priming and pipeline restart.  Pick the chunk count
+// that maximises useful work over that estimate (chunks of at least max(NG+1, 6) planes).
 static void choose_chunks(MarchPlan& m, int n2, int ng, int slots) {
   const char* zc_env = std::getenv("HR_TUNE_ZC");  // tuning knob: planes per chunk
   if (zc_env && std::atoi(zc_env) > 0) {
@@ -473,17 +473,21 @@ static void choose_chunks(MarchPlan& m, int n2, int ng, int slots) {
     return;
   }
   const int ntiles = m.ntx * m.nty;
-  const int min_zc = 2 * ng > 6 ? 2 * ng : 6;
+  const int min_zc = ng + 1 > 6 ? ng + 1 : 6;
   int best_nzc = 1;
   double best = -1.0;
   for (int nzc = 1; nzc <= n2; ++nzc) {
     const int zc = (n2 + nzc - 1) / nzc;
-    if (nzc > 1 && zc < min_zc) break;
     if ((n2 + zc - 1) / zc != nzc) continue;  // not a distinct chunking
-    const long long items = (long long)ntiles * nzc;
-    const long long rounds = (items + slots - 1) / slots;
-    // time ~ rounds x (zc + priming); useful work ~ items x zc / slots
-    const double eff = ((double)items * zc / slots) / ((double)rounds * (zc + 0.25 * ng + 1.0));
+    const double items = (double)ntiles * nzc;
+    const double rounds = items / slots;
+    // short chunks only while there are idle SMs to give them to (small grids: latency regime,
+    // where an item's fixed cost is about three planes' worth)
+    if (zc < min_zc && (rounds > 1.0 || zc < 2)) break;
+    const double prime = rounds < 1.0 ? 3.0 : 1.0;
+    const double useful = (double)ntiles * n2 / slots;
+    const double time = (rounds < 1.0 ? 1.0 : rounds) * (zc + prime) + (rounds > 1.0 ? zc + prime : 0.0);
+    const double eff = useful / time;
     if (eff > best + 1e-9) {
       best = eff;
       best_nzc = nzc;

@@ -271,7 +271,12 @@ __global__ void __launch_bounds__((TW / VX) * BY,
   double num = 0.0, den = 0.0;
   unsigned n_cons = 0;  // planes consumed so far by this CTA: slot = n % RING, parity = n / RING
 
-  for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
+  // The first item of a CTA is its block index; further items are handed out by an atomic counter
+  // (items differ in cost: boundary tiles also write ghost images), except for the residual,
+  // whose per-CTA partial sums must not depend on timing (C16: fixed reduction order).
+  __shared__ int s_item;
+  int item = blockIdx.x;
+  while (item < n_items) {
     const int chunk = item / ntiles;
     const int tile_id = item - chunk * ntiles;
     const int zi = chunk * plan.zc;
@@ -461,6 +466,21 @@ __global__ void __launch_bounds__((TW / VX) * BY,
         }
 #undef HR_W
       }
+    }
+    if constexpr (STAGE == 5) {
+      item += gridDim.x;
+    } else {
+      __syncthreads();  // all threads are done with this item (and with s_item)
+      if (tid == 0) s_item = (int)gridDim.x + atomicAdd(plan.counters + 2 * STAGE, 1);
+      __syncthreads();
+      item = s_item;
+    }
+  }
+  if constexpr (STAGE != 5) {
+    // the last CTA to leave the item loop re-arms the counters for the next launch of this stage
+    if (tid == 0 && atomicAdd(plan.counters + 2 * STAGE + 1, 1) == (int)gridDim.x - 1) {
+      plan.counters[2 * STAGE] = 0;
+      plan.counters[2 * STAGE + 1] = 0;
     }
   }
 
