@@ -81,14 +81,19 @@ typedef struct {
   double cfl;            /* dt = cfl * ds_min over interior points (C9)                       */
   double c_min;          /* wave-speed normalisation: c(x) = c_min ds(x)/ds_min (C9)          */
   int32_t device;        /* CUDA device ordinal                                               */
-  int32_t variant;       /* kernel arrangement: 0 = default (fused, tiled);
-                            1 = paper arrangement ablation (one thread per point, direct
-                            global loads, k stored, separate RK kernel)     */
+  int32_t variant;       /* kernel arrangement: 0 = default (fused RHS + radiation + RK combine +
+                            ghost images in one TMA-fed marching kernel per substep);
+                            2 = direct-load fused kernel (one thread per point, stencil through
+                            L1/L2) + list-driven inner fill, kept for comparison;
+                            1 = reserved for the paper-arrangement ablation (k stored, separate
+                            RK kernel), HR_ERR_UNSUPPORTED for now            */
   void* stream;          /* cudaStream_t owned by the caller; must outlive the solver         */
 } hr_params;
 
 /* Bytes of device workspace hr_create needs for these parameters (10 grid functions, the
- * (i0,i1) coefficient planes, the boundary lists, reduction scratch). */
+ * (i0,i1) coefficient planes, the boundary lists, reduction scratch).  Inside
+ * the workspace every grid function is stored with rows padded to 128-byte lines; the layout
+ * above is what crosses this boundary (hr_get_u, hr_set_state, hr_eval_rhs convert). */
 HR_API hr_status hr_workspace_bytes(const hr_params* p, size_t* bytes);
 
 /* Alg. 1 l.2-7: coordinate arrays, reference-metric factor planes, wave speed
@@ -103,8 +108,9 @@ HR_API hr_status hr_create(const hr_params* p, void* workspace_dev, size_t works
 HR_API hr_status hr_destroy(hr_solver* s);
 
 /* Alg. 1 l.12-16 x n_steps: n_steps classic RK4 steps (C15), each four substeps of
- * [fused RHS (Eq. 5) + radiation condition at the outer points (C13) + RK combine] followed by the
- * inner-boundary fill (C14).  Enqueues on the stream and returns; n_steps >= 0. */
+ * [RHS (Eq. 5) + radiation condition at the outer points (C13) + RK combine + inner-boundary
+ * fill (C14)] -- one kernel launch per substep in the default arrangement.  Enqueues on the
+ * stream and returns; n_steps >= 0. */
 HR_API hr_status hr_step(hr_solver* s, int64_t n_steps);
 
 /* Alg. 1 l.9-11: H = lap u + S (psi_BL + u)^-7 at interior points and its grid L2 norm in the
@@ -162,7 +168,8 @@ HR_API hr_status hr_host_setup(const hr_params* p, double* dt, double* dsmin, in
  * launches of the same kernels hr_step uses, each bracketed by a CUDA event pair on the solver's
  * stream, preceded per step by one residual evaluation (Alg. 1 l.9-11) if with_residual != 0.
  * ms6 (host pointer, 6 doubles) receives the mean milliseconds per RK4 step spent in
- * { fused substep kernel of stage 1, 2, 3, 4, the four inner fills together, residual }.
+ * { fused substep kernel of stage 1, 2, 3, 4, the four inner fills together (0 in the default
+ * arrangement, whose substep kernel writes the ghost images itself), residual }.
  * Synchronises the stream. */
 HR_API hr_status hr_profile_step(hr_solver* s, int64_t n_steps, int32_t with_residual, double* ms6);
 

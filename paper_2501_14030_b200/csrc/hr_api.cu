@@ -683,7 +683,8 @@ hr_status hr_profile_step(hr_solver* s, int64_t n_steps, int32_t with_residual, 
   if (!s || !ms6) return fail(HR_ERR_INVALID_ARG, "NULL argument");
   if (n_steps < 1 || n_steps > 4096) return fail(HR_ERR_INVALID_ARG, "n_steps must be in 1..4096");
   // one event pair per launch; elapsed times are read after a single synchronisation at the end
-  const int per_step = 8 + (with_residual ? 1 : 0);
+  const bool has_fill = hrk_launches_per_substep(s) == 2;  // variant 2 only: separate inner fill
+  const int per_step = 4 + (has_fill ? 4 : 0) + (with_residual ? 1 : 0);
   std::vector<cudaEvent_t> ev((size_t)n_steps * per_step * 2, nullptr);
   struct Cleanup {
     std::vector<cudaEvent_t>& ev;
@@ -701,9 +702,11 @@ hr_status hr_profile_step(hr_solver* s, int64_t n_steps, int32_t with_residual, 
       HR_CUDA(cudaEventRecord(ev[k++], s->stream));
       HR_CUDA(hrk_substep_main(s, stage));
       HR_CUDA(cudaEventRecord(ev[k++], s->stream));
-      HR_CUDA(cudaEventRecord(ev[k++], s->stream));
-      HR_CUDA(hrk_substep_fill(s, stage));
-      HR_CUDA(cudaEventRecord(ev[k++], s->stream));
+      if (has_fill) {
+        HR_CUDA(cudaEventRecord(ev[k++], s->stream));
+        HR_CUDA(hrk_substep_fill(s, stage));
+        HR_CUDA(cudaEventRecord(ev[k++], s->stream));
+      }
     }
   }
   HR_CUDA(cudaStreamSynchronize(s->stream));
@@ -719,7 +722,7 @@ hr_status hr_profile_step(hr_solver* s, int64_t n_steps, int32_t with_residual, 
     if (with_residual) { HR_CUDA(el(k, acc[5])); k += 2; }
     for (int stage = 1; stage <= 4; ++stage) {
       HR_CUDA(el(k, acc[stage - 1])); k += 2;
-      HR_CUDA(el(k, acc[4])); k += 2;
+      if (has_fill) { HR_CUDA(el(k, acc[4])); k += 2; }
     }
   }
   for (int i = 0; i < 6; ++i) ms6[i] = acc[i] / (double)n_steps;
