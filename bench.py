@@ -320,6 +320,7 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-f32", action="store_true")
+    ap.add_argument("--no-also", action="store_true", help="skip the extra config1/config2 timings")
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"],
                     help="precision of the headline leg (f32: for profiling the fp32 kernels alone)")
     args = ap.parse_args()
@@ -387,6 +388,25 @@ def main():
         s32.close()
         del s32
 
+    # the smaller configs of BASELINE.json on the same box (rank 0, N = 1 only): L2-resident grids where
+    # the step is bound by launch latency and the serial plane march, reported beside the headline
+    also = None
+    if world == 1 and args.workload == "config3" and not args.no_also:
+        also = {}
+        for other in ("config1", "config2"):
+            po = workload(other)
+            To = [x + po["fd_order"] for x in po["n"]]
+            nto = To[0] * To[1] * To[2]
+            nio = po["n"][0] * po["n"][1] * po["n"][2]
+            entry = {"n_interior": list(po["n"]), "fd_order": po["fd_order"],
+                     "l2": "L2 flushed between timed steps" if 10 * nto * 8 <= 126e6 else "larger than L2"}
+            for dt, w in (("f64", 8), ("f32", 4)):
+                sec, so = time_resident(torch, hr, po, dt, 20, 3, None, 10 * nto * w <= 126e6)
+                entry[dt] = {"value": nio * 4 * 20 / sec, "unit": UNIT, "ms_per_step": 1e3 * sec / 20}
+                so.close()
+                del so
+            also[other] = entry
+
     if dist is not None:
         dist.barrier()
     if rank != 0:
@@ -400,6 +420,8 @@ def main():
             "config": config_dict(p, name, world), "clocks": clocks, "e2e": e2e,
             "gpu_launches": launches_per_step * args.steps, "roofline": roof, "f32": f32,
             "library": hr.hr_version()}
+    if also is not None:
+        line["also"] = also
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(p, name)
     print(json.dumps(line), flush=True)

@@ -85,8 +85,9 @@ typedef struct {
                             ghost images in one TMA-fed marching kernel per substep);
                             2 = direct-load fused kernel (one thread per point, stencil through
                             L1/L2) + list-driven inner fill, kept for comparison;
-                            1 = reserved for the paper-arrangement ablation (k stored, separate
-                            RK kernel), HR_ERR_UNSUPPORTED for now            */
+                            1 = the paper's arrangement as an ablation: one thread per point,
+                            block (32, NGHOSTS, 1), RHS -> BC -> RK as separate kernels with k
+                            stored in HBM                              */
   void* stream;          /* cudaStream_t owned by the caller; must outlive the solver         */
 } hr_params;
 

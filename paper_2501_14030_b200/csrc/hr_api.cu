@@ -53,7 +53,7 @@ hr_status validate(const hr_params* p) {
     return fail(HR_ERR_UNSUPPORTED, "coord %d unknown", p->coord);
   if (p->dtype != HR_F64 && p->dtype != HR_F32)
     return fail(HR_ERR_UNSUPPORTED, "dtype %d unknown", p->dtype);
-  if (p->variant != 0 && p->variant != 2)
+  if (p->variant < 0 || p->variant > 2)
     return fail(HR_ERR_UNSUPPORTED, "variant %d unknown", p->variant);
   const int ng = p->fd_order / 2;
   for (int a = 0; a < 3; ++a)
@@ -683,7 +683,7 @@ hr_status hr_profile_step(hr_solver* s, int64_t n_steps, int32_t with_residual, 
   if (!s || !ms6) return fail(HR_ERR_INVALID_ARG, "NULL argument");
   if (n_steps < 1 || n_steps > 4096) return fail(HR_ERR_INVALID_ARG, "n_steps must be in 1..4096");
   // one event pair per launch; elapsed times are read after a single synchronisation at the end
-  const bool has_fill = hrk_launches_per_substep(s) == 2;  // variant 2 only: separate inner fill
+  const bool has_fill = hrk_launches_per_substep(s) >= 2;  // variants 1, 2: launches after the main kernel
   const int per_step = 4 + (has_fill ? 4 : 0) + (with_residual ? 1 : 0);
   std::vector<cudaEvent_t> ev((size_t)n_steps * per_step * 2, nullptr);
   struct Cleanup {

@@ -193,6 +193,74 @@ __global__ void __launch_bounds__(DBX* DBY)
 }
 
 // ------------------------------------------------------------------------------------------
+// Variant 1, the paper's arrangement as an ablation: one thread
+// per point with block (32, NGHOSTS, 1), no shared memory, RHS -> BC -> RK as separate kernels
+// with k stored in HBM (buffer B) and re-read by the RK kernel.  (The reference-metric factors
+// still come from the (i0,i1) planes; the paper evaluates CSE'd expressions instead.)
+// ------------------------------------------------------------------------------------------
+template <typename T, int NG>
+__global__ void __launch_bounds__(32 * NG)
+    k_paper_rhs(const __grid_constant__ HrGrid g, const __grid_constant__ StepArgs<T> a) {
+  const int i0 = NG + blockIdx.x * 32 + threadIdx.x;
+  const int i1 = NG + blockIdx.y * NG + threadIdx.y;
+  const int i2 = NG + blockIdx.z;
+  if (i0 >= g.n0 + NG || i1 >= g.n1 + NG) return;
+  const int64_t c = g.off0 + i0 + g.s1 * i1 + g.s2 * i2;
+  const int64_t q = i0 + (int64_t)g.T0 * i1;
+  const T uc = a.in_u[c], vc = a.in_v[c];
+  const T lap = laplacian_direct<T, NG>(a.in_u, c, g.s1, g.s2, uc, a.L00[q], a.L11[q], a.L22[q],
+                                        a.L0[q], a.L1[q]);
+  a.out_u[c] = vc - a.eta * uc;
+  a.out_v[c] = a.C2[q] * (lap + a.S[c] * pow_m7(a.psi[c] + uc));
+}
+
+template <typename T, int NG>
+__global__ void __launch_bounds__(256)
+    k_paper_bc_outer(const __grid_constant__ HrGrid g, const __grid_constant__ StepArgs<T> a) {
+  const int m = blockIdx.x * 256 + threadIdx.x;
+  if (m >= NG * g.n1 * g.n2) return;
+  const int j = m % NG;
+  const int r = m / NG;
+  const int i1 = NG + r % g.n1, i2 = NG + r / g.n1;
+  const int64_t c = g.off0 + (g.n0 + NG + j) + g.s1 * i1 + g.s2 * i2;
+  const int qo = j + NG * i1;
+  const T r0 = a.RAD0[qo], r1 = a.RAD1[qo], ri = a.RADI[qo];
+  a.out_u[c] = radiation_k(a.in_u, c, g.s1, r0, r1, ri);
+  a.out_v[c] = radiation_k(a.in_v, c, g.s1, r0, r1, ri);
+}
+
+// RK combine over all stored points (ghosts included, as Alg. 1 l.15 has it): k = (ku, kv) from
+// HBM; stage 1-3 write the next stage state (in place in A) and the running sum, stage 4 writes Y.
+template <typename T, int STAGE>
+__global__ void __launch_bounds__(256)
+    k_paper_rk(int64_t n, T dt, const T* __restrict__ ku, const T* __restrict__ kv,
+               T* __restrict__ y_u, T* __restrict__ y_v, T* __restrict__ st_u,
+               T* __restrict__ st_v, T* __restrict__ acc_u, T* __restrict__ acc_v) {
+  const int64_t c = (int64_t)blockIdx.x * 256 + threadIdx.x;
+  if (c >= n) return;
+  T yu = T(0), yv = T(0), au = T(0), av = T(0);
+  if constexpr (STAGE <= 3) {
+    yu = y_u[c];
+    yv = y_v[c];
+  }
+  if constexpr (STAGE >= 2) {
+    au = acc_u[c];
+    av = acc_v[c];
+  }
+  T wu, wv, nu, nv;
+  rk_values<T, STAGE>(dt, ku[c], kv[c], yu, yv, yu, yv, au, av, wu, wv, nu, nv);
+  if constexpr (STAGE <= 3) {
+    st_u[c] = wu;
+    st_v[c] = wv;
+    acc_u[c] = nu;
+    acc_v[c] = nv;
+  } else {
+    y_u[c] = wu;
+    y_v[c] = wv;
+  }
+}
+
+// ------------------------------------------------------------------------------------------
 // a3: inner ghosts through the precomputed index map (C14), parity +1
 // ------------------------------------------------------------------------------------------
 template <typename T>
@@ -411,6 +479,71 @@ cudaError_t launch_substep_direct(const hr_solver* s, int stage, void* ku, void*
     default: k_substep_direct<T, NG, 4><<<grid, block, 0, s->stream>>>(g, a); break;
   }
   return cudaGetLastError();
+}
+
+// ---- paper arrangement (variant 1) ----
+// stage s: k = RHS(in) into B (in = Y for stage 1, else the stage state A); (ku, kv) given for eval
+template <typename T>
+StepArgs<T> make_args_paper(const hr_solver* s, int stage, void* ku, void* kv) {
+  StepArgs<T> r = make_args<T>(s, 0, ku ? ku : s->a.B[0], kv ? kv : s->a.B[1]);
+  if (stage >= 2) {
+    r.in_u = static_cast<T*>(s->a.A[0]);
+    r.in_v = static_cast<T*>(s->a.A[1]);
+  }
+  return r;
+}
+
+template <typename T, int NG>
+cudaError_t launch_paper_rhs(const hr_solver* s, int stage, void* ku, void* kv) {
+  const HrGrid& g = s->g;
+  const StepArgs<T> a = make_args_paper<T>(s, stage, ku, kv);
+  const dim3 block(32, NG, 1);
+  const dim3 grid((g.n0 + 31) / 32, (g.n1 + NG - 1) / NG, g.n2);
+  k_paper_rhs<T, NG><<<grid, block, 0, s->stream>>>(g, a);
+  return cudaGetLastError();
+}
+
+template <typename T, int NG>
+cudaError_t launch_paper_bc_outer(const hr_solver* s, int stage, void* ku, void* kv) {
+  const HrGrid& g = s->g;
+  const StepArgs<T> a = make_args_paper<T>(s, stage, ku, kv);
+  const int n = NG * g.n1 * g.n2;
+  k_paper_bc_outer<T, NG><<<(n + 255) / 256, 256, 0, s->stream>>>(g, a);
+  return cudaGetLastError();
+}
+
+template <typename T>
+cudaError_t launch_paper_rk(const hr_solver* s, int stage) {
+  const HrArrays& a = s->a;
+  auto P = [](void* p) { return static_cast<T*>(p); };
+  const int64_t n = s->g.npad;
+  const int blocks = (int)((n + 255) / 256);
+  const T dt = (T)s->dt;
+#define HR_RK(ST)                                                                                \
+  k_paper_rk<T, ST><<<blocks, 256, 0, s->stream>>>(n, dt, P(a.B[0]), P(a.B[1]), P(a.Y[0]),      \
+                                                    P(a.Y[1]), P(a.A[0]), P(a.A[1]), P(a.ACC[0]), \
+                                                    P(a.ACC[1]))
+  switch (stage) {
+    case 1: HR_RK(1); break;
+    case 2: HR_RK(2); break;
+    case 3: HR_RK(3); break;
+    default: HR_RK(4); break;
+  }
+#undef HR_RK
+  return cudaGetLastError();
+}
+
+template <typename T>
+cudaError_t dispatch_paper(const hr_solver* s, int what, int stage, void* ku, void* kv) {
+#define HR_NGCASE(N)                                                          \
+  case N:                                                                     \
+    return what == 0 ? launch_paper_rhs<T, N>(s, stage, ku, kv)               \
+                     : launch_paper_bc_outer<T, N>(s, stage, ku, kv);
+  switch (s->g.ng) {
+    HR_NGCASE(1) HR_NGCASE(2) HR_NGCASE(3) HR_NGCASE(4) HR_NGCASE(5) HR_NGCASE(6)
+  }
+#undef HR_NGCASE
+  return cudaErrorInvalidValue;
 }
 
 // ---- marching arrangement (variant 0) ----
@@ -633,7 +766,7 @@ cudaError_t launch_residual(const hr_solver* s, int mode, double* out2) {
   const HrArrays& a = s->a;
   int64_t nb;
   cudaError_t e;
-  if (s->p.variant == 2) {
+  if (s->p.variant != 0) {
     auto P = [](void* p) { return static_cast<const T*>(p); };
     const dim3 block(RBX, RBY, 1);
     const dim3 grid((g.n0 + RBX - 1) / RBX, (g.n1 + RBY - 1) / RBY, g.n2);
@@ -682,7 +815,7 @@ MarchPlan hrk_make_plan(const int32_t n[3], int ng, int coord, int dtype) {
 }
 
 cudaError_t hrk_prepare(hr_solver* s) {
-  if (s->p.variant == 2) return cudaSuccess;
+  if (s->p.variant != 0) return cudaSuccess;
   return s->p.dtype == HR_F64 ? prepare_march_ng<double>(s) : prepare_march_ng<float>(s);
 }
 
@@ -694,6 +827,7 @@ int hrk_max_partials(const int32_t n[3], int ng) {
 }
 
 int hrk_launches_per_substep(const hr_solver* s) {
+  if (s->p.variant == 1) return 4;  // RHS, BC outer, BC inner, RK
   if (s->p.variant == 2) return s->g.n_inner > 0 ? 2 : 1;
   return 1;
 }
@@ -731,11 +865,21 @@ cudaError_t hrk_inner_fill(const hr_solver* s, void* fu, void* fv) {
 }
 
 cudaError_t hrk_substep_main(const hr_solver* s, int stage) {
+  if (s->p.variant == 1)  // the RHS kernel alone; BC and RK follow in hrk_substep_fill
+    return s->p.dtype == HR_F64 ? dispatch_paper<double>(s, 0, stage, nullptr, nullptr)
+                                : dispatch_paper<float>(s, 0, stage, nullptr, nullptr);
   return s->p.dtype == HR_F64 ? dispatch_substep<double>(s, stage, nullptr, nullptr)
                               : dispatch_substep<float>(s, stage, nullptr, nullptr);
 }
 
 cudaError_t hrk_substep_fill(const hr_solver* s, int stage) {
+  if (s->p.variant == 1) {  // Alg. 1 l.14-15 as separate kernels: BC (outer, inner) on k, then RK
+    cudaError_t e = s->p.dtype == HR_F64 ? dispatch_paper<double>(s, 1, stage, nullptr, nullptr)
+                                         : dispatch_paper<float>(s, 1, stage, nullptr, nullptr);
+    if (e != cudaSuccess) return e;
+    if ((e = hrk_inner_fill(s, s->a.B[0], s->a.B[1])) != cudaSuccess) return e;
+    return s->p.dtype == HR_F64 ? launch_paper_rk<double>(s, stage) : launch_paper_rk<float>(s, stage);
+  }
   if (s->p.variant != 2) return cudaSuccess;  // the marching kernel writes the ghost images itself
   // a3 on the array this stage wrote (bitwise equivalent to filling k, C15)
   void* const* out = (stage == 1 || stage == 3) ? s->a.A : (stage == 2 ? s->a.B : s->a.Y);
@@ -749,6 +893,15 @@ cudaError_t hrk_substep(const hr_solver* s, int stage) {
 }
 
 cudaError_t hrk_eval_rhs(const hr_solver* s, void* ku, void* kv) {
+  if (s->p.variant == 1) {
+    cudaError_t e1 = s->p.dtype == HR_F64 ? dispatch_paper<double>(s, 0, 1, ku, kv)
+                                          : dispatch_paper<float>(s, 0, 1, ku, kv);
+    if (e1 != cudaSuccess) return e1;
+    e1 = s->p.dtype == HR_F64 ? dispatch_paper<double>(s, 1, 1, ku, kv)
+                              : dispatch_paper<float>(s, 1, 1, ku, kv);
+    if (e1 != cudaSuccess) return e1;
+    return hrk_inner_fill(s, ku, kv);
+  }
   cudaError_t e = s->p.dtype == HR_F64 ? dispatch_substep<double>(s, 0, ku, kv)
                                        : dispatch_substep<float>(s, 0, ku, kv);
   if (e != cudaSuccess) return e;

@@ -333,3 +333,30 @@ def test_largest_sweep_point_sampled(hr):
     m = o.interior_mask()
     assert relmax(kv[m], okv[m]) <= 1e-5 and relmax(ku[m], oku[m]) <= 1e-5
     s.close()
+
+
+@pytest.mark.parametrize("variant", [1, 2], ids=["paper_arrangement", "direct_fused"])
+@pytest.mark.parametrize("name,params", [SMALL[0], SMALL[3], SMALL[5]], ids=[SMALL[0][0], SMALL[3][0], SMALL[5][0]])
+def test_other_arrangements_match_oracle(hr, name, params, variant):
+    """The comparison arrangements (variant 1: the paper's RHS -> BC -> RK kernels with k in HBM,
+    SURVEY.md f4; variant 2: round-1a direct-load fused kernel) meet the same bars as the default."""
+    o = Oracle(params)
+    for dtype in ("f64", "f32"):
+        s = hr.Solver(params, dtype=dtype, variant=variant)
+        u0, v0 = consistent_state(o, 5, dtype)
+        s.hr_set_state(u0, v0)
+        ku, kv = s.hr_eval_rhs()
+        oku, okv = o.rhs(u0.astype(np.float64), v0.astype(np.float64))
+        assert relmax(ku, oku) <= TOL_RHS[dtype] and relmax(kv, okv) <= TOL_RHS[dtype]
+        s.close()
+    s = hr.Solver(params, variant=variant)
+    z = np.zeros(o.ntot)
+    s.hr_step(20)
+    ou, ov = o.step(z, z, 20)
+    for mode in (0, 1):
+        r, ro = s.hr_residual(mode), o.residual(ou, mode)
+        assert abs(r - ro) <= 1e-10 * ro, (mode, r, ro)
+    u = s.hr_get_u()
+    dst, src, _ = o.bc_lists()
+    assert np.array_equal(u[dst], u[src])
+    s.close()
