@@ -126,6 +126,23 @@ HR_API hr_status hr_residual_ex(hr_solver* s, int32_t mode, double* out3);
  * pointer); no host synchronisation. */
 HR_API hr_status hr_residual_async(hr_solver* s, int32_t mode, double* out2_dev);
 
+/* Alg. 1 l.8-18, the relaxation loop with its stopping criterion (C18): repeat
+ * { residual (l.9-11); check_every RK4 steps (l.12-16) } until the residual norm (mode 0 or 1, C16)
+ * is <= tol or max_steps steps have been taken.  The loop never stalls the device: each residual
+ * is reduced on the device, copied to pinned host memory asynchronously, and tested by the host one
+ * block later, while the next block of steps is already enqueued (PAPER.md:188 overlaps the norm
+ * with the device-to-host copies in the same way).  Consequently the state has advanced one
+ * block (check_every steps) past the residual that met tol; the last history entry is the
+ * residual of the returned state.
+ *   steps_done        (host, optional) RK4 steps enqueued in total
+ *   final_residual    (host, optional) residual norm of the state on return (synchronous)
+ *   history, history_cap, n_history (host, optional) the residuals tested, one per block, in
+ *                     order: history[j] = norm after j * check_every steps
+ * max_steps >= 0, check_every >= 1, tol >= 0 (0: run max_steps).  Synchronises the stream. */
+HR_API hr_status hr_relax(hr_solver* s, int64_t max_steps, int64_t check_every, double tol, int32_t mode,
+                          int64_t* steps_done, double* final_residual, double* history,
+                          int64_t history_cap, int64_t* n_history);
+
 /* Copy the current u (or v), N_tot scalars of the solver's dtype in the layout above, ghost
  * points included, to dst (device pointer if dst_on_device != 0, else host pointer).
  * bytes must equal N_tot * sizeof(scalar).  Synchronises the stream. */

@@ -67,6 +67,8 @@ _SIGS = {
     "hr_residual": [_vp, C.POINTER(C.c_double)],
     "hr_residual_ex": [_vp, _i32, C.POINTER(C.c_double)],
     "hr_residual_async": [_vp, _i32, _vp],
+    "hr_relax": [_vp, _i64, _i64, C.c_double, _i32, C.POINTER(_i64), C.POINTER(C.c_double), _vp, _i64,
+                 C.POINTER(_i64)],
     "hr_get_u": [_vp, _vp, _sz, _i32],
     "hr_get_v": [_vp, _vp, _sz, _i32],
     "hr_set_state": [_vp, _vp, _vp, _i32],
@@ -278,6 +280,16 @@ class Solver:
         _check(lib.hr_get_bc_lists(self._h, _vp(dst.ctypes.data), _vp(src.ctypes.data), C.byref(ni),
                                    _vp(out.ctypes.data), C.byref(no)))
         return dst, src, out
+
+    def hr_relax(self, max_steps: int, check_every: int, tol: float, mode=0):
+        """Alg. 1's relaxation loop with stopping criterion -> (steps done, final residual, history)."""
+        cap = int(max_steps) // max(1, int(check_every)) + 3
+        hist = np.zeros(cap, dtype=np.float64)
+        done, nh, res = _i64(0), _i64(0), C.c_double(0.0)
+        _check(lib.hr_relax(self._h, _i64(int(max_steps)), _i64(int(check_every)), C.c_double(float(tol)),
+                            _i32(int(mode)), C.byref(done), C.byref(res), _vp(hist.ctypes.data), _i64(cap),
+                            C.byref(nh)))
+        return int(done.value), float(res.value), hist[:min(cap, int(nh.value))].copy()
 
     def hr_profile_step(self, n_steps: int, with_residual=True):
         """Mean ms per RK4 step in {stage 1..4 fused kernel, inner fills, residual}."""

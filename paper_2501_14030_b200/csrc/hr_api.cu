@@ -580,6 +580,62 @@ hr_status hr_residual_ex(hr_solver* s, int32_t mode, double* out3) {
   return HR_OK;
 }
 
+hr_status hr_relax(hr_solver* s, int64_t max_steps, int64_t check_every, double tol, int32_t mode,
+                   int64_t* steps_done, double* final_residual, double* history,
+                   int64_t history_cap, int64_t* n_history) {
+  if (!s) return fail(HR_ERR_INVALID_ARG, "solver is NULL");
+  if (max_steps < 0 || check_every < 1 || !(tol >= 0) || (mode != 0 && mode != 1))
+    return fail(HR_ERR_INVALID_ARG, "need max_steps >= 0, check_every >= 1, tol >= 0, mode 0 or 1");
+  if (history && history_cap < 0) return fail(HR_ERR_INVALID_ARG, "history_cap < 0");
+  // two pinned slots and two events: the host tests block k-1 while block k runs
+  struct Pinned {
+    double* h = nullptr;
+    cudaEvent_t ev[2] = {nullptr, nullptr};
+    ~Pinned() {
+      if (h) cudaFreeHost(h);
+      for (cudaEvent_t e : ev) if (e) cudaEventDestroy(e);
+    }
+  } pin;
+  HR_CUDA(cudaHostAlloc(reinterpret_cast<void**>(&pin.h), 4 * sizeof(double), cudaHostAllocDefault));
+  for (auto& e : pin.ev) HR_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+  double* dev = s->a.result2 + 2;  // device slots {num, den} x 2 behind hr_residual's own pair
+  int64_t done = 0, nh = 0, k = 0;
+  bool met = false;
+  auto test_block = [&](int64_t kk) -> hr_status {
+    HR_CUDA(cudaEventSynchronize(pin.ev[kk & 1]));
+    const double r = std::sqrt(pin.h[2 * (kk & 1)] / pin.h[2 * (kk & 1) + 1]);
+    if (history && nh < history_cap) history[nh] = r;
+    ++nh;
+    if (tol > 0 && r <= tol) met = true;
+    return HR_OK;
+  };
+  while (true) {
+    HR_CUDA(hrk_residual(s, mode, dev + 2 * (k & 1)));
+    HR_CUDA(cudaMemcpyAsync(pin.h + 2 * (k & 1), dev + 2 * (k & 1), 2 * sizeof(double),
+                            cudaMemcpyDeviceToHost, s->stream));
+    HR_CUDA(cudaEventRecord(pin.ev[k & 1], s->stream));
+    if (k > 0) HR_TRY(test_block(k - 1));  // long complete: the device is busy with block k-1
+    const int64_t n = max_steps - done < check_every ? max_steps - done : check_every;
+    if (met || n <= 0) {
+      HR_TRY(test_block(k));  // the residual of the final state closes the history
+      break;
+    }
+    HR_TRY(hr_step(s, n));
+    done += n;
+    ++k;
+  }
+  if (steps_done) *steps_done = done;
+  if (n_history) *n_history = nh;
+  if (final_residual) {
+    double o3[3];
+    HR_TRY(hr_residual_ex(s, mode, o3));
+    *final_residual = o3[0];
+  } else {
+    HR_CUDA(cudaStreamSynchronize(s->stream));
+  }
+  return HR_OK;
+}
+
 hr_status hr_residual(hr_solver* s, double* out) {
   if (!s || !out) return fail(HR_ERR_INVALID_ARG, "NULL argument");
   double o3[3];

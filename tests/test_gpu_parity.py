@@ -360,3 +360,36 @@ def test_other_arrangements_match_oracle(hr, name, params, variant):
     dst, src, _ = o.bc_lists()
     assert np.array_equal(u[dst], u[src])
     s.close()
+
+
+def test_relaxation_loop_with_stopping_criterion(hr):
+    """hr_relax (Alg. 1 l.8-18): residual history equals the oracle's, block by block, and the loop stops
+    one block after the first residual <= tol (the host tests a residual while the next block runs)."""
+    params = W.config(0)
+    o = Oracle(params)
+    every = 20
+    z = np.zeros(o.ntot)
+    ou, ov = z.copy(), z.copy()
+    ref = [o.residual(ou, 0)]
+    for _ in range(10):
+        ou, ov = o.step(ou, ov, every)
+        ref.append(o.residual(ou, 0))
+    ref = np.array(ref)
+    assert np.all(np.diff(ref[3:]) < 0)  # decaying after the transient (P11), so a threshold is meaningful
+    j = 6
+    tol = float(np.sqrt(ref[j] * ref[j - 1]))  # between two checks: the decision is not borderline
+    s = hr.Solver(params)
+    done, res, hist = s.hr_relax(10_000, every, tol, 0)
+    assert done == (j + 1) * every, (done, j)
+    assert len(hist) == j + 2
+    assert np.all(np.abs(hist - ref[:j + 2]) <= 1e-10 * ref[:j + 2])
+    assert res == hist[-1]
+    # tol = 0 runs max_steps (ragged last block)
+    s2 = hr.Solver(params)
+    done2, res2, hist2 = s2.hr_relax(50, every, 0.0, 0)
+    assert done2 == 50 and len(hist2) == 4
+    s3 = hr.Solver(params)
+    s3.hr_step(50)
+    assert res2 == s3.hr_residual(0)
+    for x in (s, s2, s3):
+        x.close()
