@@ -187,6 +187,23 @@ def run_reference(args, p, name):
 
 
 # ------------------------------------------------------------------------------------------------
+# N > 1: replicas only.  No data-path collective: the only exchange is the
+# maximum over ranks of the device time; value = all ranks' units / that time.
+# ------------------------------------------------------------------------------------------------
+def max_over_ranks(torch, sec: float, dist, device) -> float:
+    if dist is None:
+        return sec
+    t = torch.tensor([sec], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def replicas_value(world: int, n_int: int, steps: int, sec_max: float) -> float:
+    """Whole-job point-substeps/s of `world` independent replicas that each did `steps` steps."""
+    return world * n_int * 4 * steps / sec_max
+
+
+# ------------------------------------------------------------------------------------------------
 # the CUDA path
 # ------------------------------------------------------------------------------------------------
 def time_resident(torch, hr, p, dtype, steps, warmup, dist, flush_l2):
@@ -233,11 +250,9 @@ def time_resident(torch, hr, p, dtype, steps, warmup, dist, flush_l2):
         ms = sum(a.elapsed_time(b) for a, b in evs)
     torch.cuda.synchronize()
     sec = ms * 1e-3
+    sec = max_over_ranks(torch, sec, dist, s.device)
     if dist is not None:
-        t = torch.tensor([sec], dtype=torch.float64, device=s.device)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
         dist.barrier()
-        sec = float(t.item())
     return sec, s
 
 
@@ -268,10 +283,7 @@ def time_e2e(torch, s, steps, warmup, dist):
     sec = max(e0.elapsed_time(e1) * 1e-3, 0.0)
     wall = time.perf_counter() - t0
     sec = max(sec, wall) if wall > 0 else sec  # host-side marshalling counts too
-    if dist is not None:
-        t = torch.tensor([sec], dtype=torch.float64, device=s.device)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        sec = float(t.item())
+    sec = max_over_ranks(torch, sec, dist, s.device)
     w = 8 if s.dtype == "f64" else 4
     return sec, 2 * s.ntot * w, 16
 
@@ -361,7 +373,7 @@ def main():
     sec64, s64 = time_resident(torch, hr, p, args.dtype, args.steps, args.warmup, dist, flush_l2)
     launches_per_step = s64.launches_per_step + 2  # + residual kernel and its final pass
     clocks = sampler.stop() if rank == 0 else None
-    value = world * n_int * 4 * args.steps / sec64
+    value = replicas_value(world, n_int, args.steps, sec64)
 
     prof64 = s64.hr_profile_step(min(args.steps, 20), True)
     roof = roofline(s64, prof64, peak, peak_src)
