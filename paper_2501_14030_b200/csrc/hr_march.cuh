@@ -51,12 +51,11 @@ __device__ __forceinline__ void mbar_fence_init() {
   asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
   asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
 }
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)),
-               "r"(bytes)
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(bar), "r"(bytes)
                : "memory");
 }
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t phase) {
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t phase) {
   uint32_t ok;
   uint32_t spins = 0;
   do {
@@ -66,16 +65,16 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t phase) {
         "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
         "selp.u32 %0, 1, 0, p;\n}\n"
         : "=r"(ok)
-        : "r"(smem_u32(bar)), "r"(phase)
+        : "r"(bar), "r"(phase)
         : "memory");
   } while (!ok);
 }
-__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, int x, int y, int z,
-                                            uint64_t* bar) {
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, int x, int y, int z,
+                                            uint32_t bar) {
   asm volatile(
       "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes "
-      "[%0], [%1, {%2, %3, %4}], [%5];\n" ::"r"(smem_u32(dst)),
-      "l"(map), "r"(x), "r"(y), "r"(z), "r"(smem_u32(bar))
+      "[%0], [%1, {%2, %3, %4}], [%5];\n" ::"r"(dst),
+      "l"(map), "r"(x), "r"(y), "r"(z), "r"(bar)
       : "memory");
 }
 
@@ -269,7 +268,10 @@ __global__ void __launch_bounds__((TW / VX) * BY,
   const int n_items = ntiles * plan.nzc;
 
   double num = 0.0, den = 0.0;
-  unsigned n_cons = 0;  // planes consumed so far by this CTA: slot = n % RING, parity = n / RING
+  // ring position of the next plane to consume, and the parity its mbarrier completes with
+  int sl = 0;
+  uint32_t par = 0;
+  const uint32_t bars_u32 = smem_u32(bars), ring_u32 = smem_u32(ring);
 
   // The first item of a CTA is its block index; further items are handed out by an atomic counter
   // (items differ in cost: boundary tiles also write ghost images), except for the residual,
@@ -289,23 +291,25 @@ __global__ void __launch_bounds__((TW / VX) * BY,
     const int nact = i1 < g.n1 + NG ? max(0, min(VX, g.n0 + NG - i0)) : 0;
     const int col = g.off0 + i0 + g.P0 * i1;  // only dereferenced if nact > 0
 
-    // one thread feeds the ring: everything plane zz needs, into slot (n_cons + d) % RING
-    auto issue = [&](int zz, unsigned n) {
-      const unsigned sl = n % RING;
-      unsigned char* base = ring + sl * SLOT_BYTES;
-      uint64_t* bar = &bars[sl];
+    // one thread feeds the ring: everything plane zz needs, into ring slot sl
+    auto issue = [&](int zz, int sl) {
+      const uint32_t base = ring_u32 + sl * SLOT_BYTES;
+      const uint32_t bar = bars_u32 + sl * 8;
       mbar_expect_tx(bar, (uint32_t)(SWA * G::SH * sizeof(T) + NS * G::BOX_BYTES));
       const int xs = g.off0 + x0;
       tma_load_3d(base, &mm.tile, xs - NGA, y0 - NG, zz, bar);
-      unsigned char* sb = base + G::TILE_BYTES;
+      const uint32_t sb = base + G::TILE_BYTES;
       tma_load_3d(sb + ST_FRONT * G::BOX_BYTES, &mm.st[ST_FRONT], xs, y0, zz + NG, bar);
 #pragma unroll
       for (int q = 1; q < NS; ++q) tma_load_3d(sb + q * G::BOX_BYTES, &mm.st[q], xs, y0, zz, bar);
     };
     if (tid == 0) {
+      int sd = sl;
 #pragma unroll
-      for (int d = 0; d < D; ++d)
-        if (z_begin + d < z_end) issue(z_begin + d, n_cons + d);
+      for (int d = 0; d < D; ++d) {
+        if (z_begin + d < z_end) issue(z_begin + d, sd);
+        if (++sd == RING) sd = 0;
+      }
     }
 
     // per-column constants
@@ -349,17 +353,22 @@ __global__ void __launch_bounds__((TW / VX) * BY,
     const int so = ly * TW + VX * lx;                                     // in a TW x BY box
     const int to = (ly + NG) * SWA + NGA + VX * lx;                       // in the halo tile
     constexpr int NE = 2 * NGV + VX;                                      // row values a thread reads
+    int cz = col + z_begin * s2;  // stored index of this thread's first point in plane z
     for (int zb = z_begin; zb < z_end; zb += UR) {
 #pragma unroll
       for (int r = 0; r < UR; ++r) {
         const int z = zb + r;
         if (z >= z_end) break;
 #define HR_W(k) p[(r + (k)) % U]
-        const unsigned sl = n_cons % RING;
         __syncthreads();  // every thread is done with plane z-1: its slot can be refilled
-        if (tid == 0 && z + D < z_end) issue(z + D, n_cons + D);
-        mbar_wait(&bars[sl], (n_cons / RING) & 1u);  // the boxes of plane z have landed
-        ++n_cons;
+        if (tid == 0 && z + D < z_end) issue(z + D, sl == 0 ? RING - 1 : sl - 1);  // (sl + D) % RING
+        mbar_wait(bars_u32 + sl * 8, par);  // the boxes of plane z have landed
+        const T* tl = reinterpret_cast<const T*>(ring + sl * SLOT_BYTES);
+        const T* sb = reinterpret_cast<const T*>(ring + sl * SLOT_BYTES + G::TILE_BYTES);
+        if (++sl == RING) {
+          sl = 0;
+          par ^= 1u;
+        }
         if (nact > 0) {
           if constexpr (UR == 1) {  // no rotation: shift the window by one plane
 #pragma unroll
@@ -367,8 +376,6 @@ __global__ void __launch_bounds__((TW / VX) * BY,
 #pragma unroll
               for (int j = 0; j < VX; ++j) p[k][j] = p[k + 1][j];
           }
-          const T* tl = reinterpret_cast<const T*>(ring + sl * SLOT_BYTES);
-          const T* sb = reinterpret_cast<const T*>(ring + sl * SLOT_BYTES + G::TILE_BYTES);
           {
             const V fr = *reinterpret_cast<const V*>(sb + ST_FRONT * (TW * BY) + so);
 #pragma unroll
@@ -440,7 +447,7 @@ __global__ void __launch_bounds__((TW / VX) * BY,
               rk_values<T, STAGE>(a.dt, ku, kv, uc, vin.v[j], yu.v[j], yv.v[j], au.v[j], av.v[j],
                                   wu.v[j], wv.v[j], nu.v[j], nv.v[j]);
             }
-            const int c = col + z * s2;
+            const int c = cz;
             if (nact == VX) {
               *reinterpret_cast<V*>(a.out_u + c) = wu;
               *reinterpret_cast<V*>(a.out_v + c) = wv;
@@ -464,6 +471,7 @@ __global__ void __launch_bounds__((TW / VX) * BY,
               scatter_vec<T, VX>(ig, a.out_u, a.out_v, wu, wv, i0, i1, z, nact, cB, cC);
           }
         }
+        cz += s2;
 #undef HR_W
       }
     }
