@@ -89,6 +89,12 @@ struct HrArrays {
 #define HR_MARCH_ROTATE 0
 #endif
 
+// 1: L2 eviction hints on the TMA loads (u: evict last, pointwise inputs: evict first).  Measured
+// on config 3: no gain (fp64 0.703 vs 0.706, fp32 0.611 vs 0.632), so off.
+#ifndef HR_MARCH_L2_HINTS
+#define HR_MARCH_L2_HINTS 0
+#endif
+
 // Planes of asynchronous look-ahead in the marching kernels.
 #ifndef HR_MARCH_D_F64
 #define HR_MARCH_D_F64 2

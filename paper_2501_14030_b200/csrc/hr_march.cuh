@@ -69,6 +69,27 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t phase) {
         : "memory");
   } while (!ok);
 }
+// L2 eviction policies for the loads: the pointwise inputs are read once per substep
+// (evict first), u is read again by the neighbouring tiles and, NG planes later, as a halo tile
+// (evict last).
+__device__ __forceinline__ uint64_t l2_policy_evict_first() {
+  uint64_t p;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;\n" : "=l"(p));
+  return p;
+}
+__device__ __forceinline__ uint64_t l2_policy_evict_last() {
+  uint64_t p;
+  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;\n" : "=l"(p));
+  return p;
+}
+__device__ __forceinline__ void tma_load_3d_hint(uint32_t dst, const CUtensorMap* map, int x, int y,
+                                                 int z, uint32_t bar, uint64_t policy) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint "
+      "[%0], [%1, {%2, %3, %4}], [%5], %6;\n" ::"r"(dst),
+      "l"(map), "r"(x), "r"(y), "r"(z), "r"(bar), "l"(policy)
+      : "memory");
+}
 __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, int x, int y, int z,
                                             uint32_t bar) {
   asm volatile(
@@ -272,6 +293,9 @@ __global__ void __launch_bounds__((TW / VX) * BY,
   int sl = 0;
   uint32_t par = 0;
   const uint32_t bars_u32 = smem_u32(bars), ring_u32 = smem_u32(ring);
+#if HR_MARCH_L2_HINTS
+  const uint64_t pol_keep = l2_policy_evict_last(), pol_stream = l2_policy_evict_first();
+#endif
 
   // The first item of a CTA is its block index; further items are handed out by an atomic counter
   // (items differ in cost: boundary tiles also write ghost images), except for the residual,
@@ -297,11 +321,20 @@ __global__ void __launch_bounds__((TW / VX) * BY,
       const uint32_t bar = bars_u32 + sl * 8;
       mbar_expect_tx(bar, (uint32_t)(SWA * G::SH * sizeof(T) + NS * G::BOX_BYTES));
       const int xs = g.off0 + x0;
+#if HR_MARCH_L2_HINTS
+      tma_load_3d_hint(base, &mm.tile, xs - NGA, y0 - NG, zz, bar, pol_keep);
+      const uint32_t sb = base + G::TILE_BYTES;
+      tma_load_3d_hint(sb + ST_FRONT * G::BOX_BYTES, &mm.st[ST_FRONT], xs, y0, zz + NG, bar, pol_keep);
+#pragma unroll
+      for (int q = 1; q < NS; ++q)
+        tma_load_3d_hint(sb + q * G::BOX_BYTES, &mm.st[q], xs, y0, zz, bar, pol_stream);
+#else
       tma_load_3d(base, &mm.tile, xs - NGA, y0 - NG, zz, bar);
       const uint32_t sb = base + G::TILE_BYTES;
       tma_load_3d(sb + ST_FRONT * G::BOX_BYTES, &mm.st[ST_FRONT], xs, y0, zz + NG, bar);
 #pragma unroll
       for (int q = 1; q < NS; ++q) tma_load_3d(sb + q * G::BOX_BYTES, &mm.st[q], xs, y0, zz, bar);
+#endif
     };
     if (tid == 0) {
       int sd = sl;
