@@ -65,23 +65,25 @@ struct HrArrays {
 };
 
 // Tiles of the marching arrangement (hr_march.cuh): TW x BY points, VX points per thread.
+// Measured on config 3 (profiles/r1b.md, r1c.md): 4-row tiles (128 threads, 4-5 CTAs per SM) beat
+// 8-row tiles (256 threads, 2-3 CTAs) by 3-4 % -- the per-plane barrier spans fewer warps.
 #ifndef HR_TW_F64
 #define HR_TW_F64 32
-#define HR_BY_F64 8
+#define HR_BY_F64 4
 #define HR_VX_F64 1
 #endif
 #ifndef HR_TW_F32
 #define HR_TW_F32 64
-#define HR_BY_F32 8
+#define HR_BY_F32 4
 #define HR_VX_F32 2
 #endif
 
 // Minimum resident CTAs per SM the marching kernels are compiled for (register cap).
 #ifndef HR_MARCH_MINB_F64
-#define HR_MARCH_MINB_F64 2
+#define HR_MARCH_MINB_F64 4
 #endif
 #ifndef HR_MARCH_MINB_F32
-#define HR_MARCH_MINB_F32 3
+#define HR_MARCH_MINB_F32 5
 #endif
 
 // 1: unroll the plane loop 2NG+1 times (rotating register window); 0: single copy + moves.

@@ -8,11 +8,13 @@
 //     compute threads spend no instructions on load addresses;
 //   * a thread owns VX consecutive points along i0 and reads / writes them as one vector
 //     (rows of the stored layout start on 128-byte lines, hr_internal.h);
-//   * the i2 stencil is a register window of 2 NG + 1 planes per point; the plane loop is
-//     unrolled 2 NG + 1 times so the window rotates through the registers without moves;
+//   * the i2 stencil is a register window of 2 NG + 1 planes per point, shifted by register
+//     moves (HR_MARCH_ROTATE = 1 unrolls the plane loop 2 NG + 1 times instead so the window
+//     rotates without moves; that copy of the loop no longer fits the 32 KB instruction cache
+//     and measured no faster);
 //   * CTAs are persistent over (chunk of planes, tile) work items in chunk-major order, so the
 //     CTAs resident at any time work on neighbouring tiles of the same planes (halo rows meet
-//     in L2);
+//     in L2); after its first item a CTA takes the next one from an atomic counter;
 //   * the reference-metric factors depend on (i0, i1) only (reading C4), so each thread loads its
 //     six coefficients once per column and keeps them in registers;
 //   * the RK combine (a4) happens in the same thread, so k never reaches HBM, and the thread that
@@ -103,8 +105,8 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map
 // interior): every ghost point whose source under the host's inner map (hr_api.cu:
 // inner_source, reading C14) is this point.  r0 = 2NG-1-j0 if j0 < 2NG else -1; cB / cC = the
 // theta-low / theta-high reflections of j1 or -1.  Each flip shifts phi by pi; phi is periodic.
-// Not inlined: few points have images, and the plane loop is unrolled 2NG+1 times -- inlining
-// this per point and per copy pushed the stage kernels out of the instruction cache.
+// Not inlined: few points have images, and inlining this into the plane loop pushed the stage
+// kernels out of the instruction cache.
 struct ImgGeom {
   int ng, n2, T1, P0, off0, sph;
 };
