@@ -595,39 +595,24 @@ cudaError_t encode_box(const hr_solver* s, CUtensorMap* map, void* base, int bw,
 }
 
 // Planes per chunk.  Work items = tiles x chunks are handed out dynamically to `slots` persistent
-// CTAs, so the run lasts about (all items' time) / slots plus one item of tail; an item costs its
-// planes plus about one plane of window priming and pipeline restart.  Pick the chunk count
-// that maximises useful work over that estimate (chunks of at least max(NG+1, 6) planes).
+// CTAs.  Measured on config 3 and on configs[4]'s sweep grids (profiles/r1c.md): chunks of 6-10
+// planes are best or within 1-2 % of best everywhere -- short items keep the hand-out balanced and
+// neighbouring tiles in step, and priming an item's 2NG-plane window costs about one plane --
+// while 32-64 planes lose up to 30 %.  So: 8 planes, shorter (down to 2) only while the grid
+// has fewer items than CTA slots (small grids, latency regime), evened out over n2.
 static void choose_chunks(MarchPlan& m, int n2, int ng, int slots) {
+  (void)ng;
   const char* zc_env = std::getenv("HR_TUNE_ZC");  // tuning knob: planes per chunk
+  int zc = 8;
   if (zc_env && std::atoi(zc_env) > 0) {
-    m.zc = std::atoi(zc_env) < n2 ? std::atoi(zc_env) : n2;
-    m.nzc = (n2 + m.zc - 1) / m.zc;
-    return;
+    zc = std::atoi(zc_env);
+  } else {
+    const long long ntiles = (long long)m.ntx * m.nty;
+    while (zc > 2 && ntiles * ((n2 + zc - 1) / zc) < slots) --zc;
   }
-  const int ntiles = m.ntx * m.nty;
-  const int min_zc = ng + 1 > 6 ? ng + 1 : 6;
-  int best_nzc = 1;
-  double best = -1.0;
-  for (int nzc = 1; nzc <= n2; ++nzc) {
-    const int zc = (n2 + nzc - 1) / nzc;
-    if ((n2 + zc - 1) / zc != nzc) continue;  // not a distinct chunking
-    const double items = (double)ntiles * nzc;
-    const double rounds = items / slots;
-    // short chunks only while there are idle SMs to give them to (small grids: latency regime,
-    // where an item's fixed cost is about three planes' worth)
-    if (zc < min_zc && (rounds > 1.0 || zc < 2)) break;
-    const double prime = rounds < 1.0 ? 3.0 : 1.0;
-    const double useful = (double)ntiles * n2 / slots;
-    const double time = (rounds < 1.0 ? 1.0 : rounds) * (zc + prime) + (rounds > 1.0 ? zc + prime : 0.0);
-    const double eff = useful / time;
-    if (eff > best + 1e-9) {
-      best = eff;
-      best_nzc = nzc;
-    }
-  }
-  m.nzc = best_nzc;
-  m.zc = (n2 + best_nzc - 1) / best_nzc;
+  if (zc > n2) zc = n2;
+  m.nzc = (n2 + zc - 1) / zc;
+  m.zc = (n2 + m.nzc - 1) / m.nzc;
 }
 
 // Persistent grid of one stage's kernel: resident CTAs per SM x SMs (never more than the work).
