@@ -114,6 +114,13 @@ HR_API hr_status hr_destroy(hr_solver* s);
  * stream and returns; n_steps >= 0. */
 HR_API hr_status hr_step(hr_solver* s, int64_t n_steps);
 
+/* PAPER.md:337-347 (N independent grids advanced together): n_steps RK4 steps of each of the n
+ * solvers, enqueued round-robin, one solver's step after the other's, each on its own solver's
+ * stream -- so the steps of different solvers overlap on the device when the solvers were created
+ * on different streams (small grids do not fill the GPU).  No data is shared between
+ * the solvers.  All solvers must live on the calling thread's current device.  Asynchronous. */
+HR_API hr_status hr_step_many(hr_solver* const* solvers, int32_t n, int64_t n_steps);
+
 /* Alg. 1 l.9-11: H = lap u + S (psi_BL + u)^-7 at interior points and its grid L2 norm in the
  * solver's residual_mode (C16), accumulated in fp64 with a fixed reduction order.
  * *out (host pointer) receives the norm; synchronises the stream. */

@@ -67,6 +67,7 @@ _SIGS = {
     "hr_residual": [_vp, C.POINTER(C.c_double)],
     "hr_residual_ex": [_vp, _i32, C.POINTER(C.c_double)],
     "hr_residual_async": [_vp, _i32, _vp],
+    "hr_step_many": [C.POINTER(_vp), _i32, _i64],
     "hr_relax": [_vp, _i64, _i64, C.c_double, _i32, C.POINTER(_i64), C.POINTER(C.c_double), _vp, _i64,
                  C.POINTER(_i64)],
     "hr_get_u": [_vp, _vp, _sz, _i32],
@@ -92,6 +93,12 @@ lib.hr_version.restype = C.c_char_p
 def _check(status):
     if status != HR_OK:
         raise HrError(status, lib.hr_last_error().decode())
+
+
+def hr_step_many(solvers, n_steps: int):
+    """n_steps RK4 steps of every Solver in `solvers`, interleaved, each on its own stream."""
+    arr = (_vp * len(solvers))(*[s._h for s in solvers])
+    _check(lib.hr_step_many(arr, _i32(len(solvers)), _i64(int(n_steps))))
 
 
 def hr_version() -> str:

@@ -560,6 +560,15 @@ hr_status hr_step(hr_solver* s, int64_t n_steps) {
   return HR_OK;
 }
 
+hr_status hr_step_many(hr_solver* const* solvers, int32_t n, int64_t n_steps) {
+  if (n < 0 || n_steps < 0 || (n > 0 && !solvers)) return fail(HR_ERR_INVALID_ARG, "bad arguments");
+  for (int32_t i = 0; i < n; ++i)
+    if (!solvers[i]) return fail(HR_ERR_INVALID_ARG, "solver %d is NULL", i);
+  for (int64_t it = 0; it < n_steps; ++it)
+    for (int32_t i = 0; i < n; ++i) HR_TRY(hr_step(solvers[i], 1));
+  return HR_OK;
+}
+
 hr_status hr_residual_async(hr_solver* s, int32_t mode, double* out2_dev) {
   if (!s || !out2_dev) return fail(HR_ERR_INVALID_ARG, "NULL argument");
   if (mode != 0 && mode != 1) return fail(HR_ERR_INVALID_ARG, "mode must be 0 or 1");

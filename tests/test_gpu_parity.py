@@ -393,3 +393,24 @@ def test_relaxation_loop_with_stopping_criterion(hr):
     assert res2 == s3.hr_residual(0)
     for x in (s, s2, s3):
         x.close()
+
+
+def test_batched_independent_grids(hr):
+    """hr_step_many: N independent solvers advanced together on their own streams give,
+    bit for bit, what each gives alone; one of them is checked against the oracle."""
+    ps = [W.sweep_point(40 + i, (32, 16, 8), "SinhSymTP", 6) for i in range(3)]
+    ps.append(W.config(0))
+    together = [hr.Solver(p) for p in ps]
+    hr.hr_step_many(together, 15)
+    for p, s in zip(ps, together):
+        alone = hr.Solver(p)
+        alone.hr_step(15)
+        assert np.array_equal(s.hr_get_u(), alone.hr_get_u()) and np.array_equal(s.hr_get_v(), alone.hr_get_v())
+        alone.close()
+    o = Oracle(ps[0])
+    z = np.zeros(o.ntot)
+    ou, _ = o.step(z, z, 15)
+    r, ro = together[0].hr_residual(0), o.residual(ou, 0)
+    assert abs(r - ro) <= 1e-10 * ro
+    for s in together:
+        s.close()
