@@ -68,6 +68,7 @@ _SIGS = {
     "hr_residual_ex": [_vp, _i32, C.POINTER(C.c_double)],
     "hr_residual_async": [_vp, _i32, _vp],
     "hr_step_many": [C.POINTER(_vp), _i32, _i64],
+    "hr_step_residual_async": [_vp, _i32, _vp],
     "hr_relax": [_vp, _i64, _i64, C.c_double, _i32, C.POINTER(_i64), C.POINTER(C.c_double), _vp, _i64,
                  C.POINTER(_i64)],
     "hr_get_u": [_vp, _vp, _sz, _i32],
@@ -226,9 +227,19 @@ class Solver:
         _check(lib.hr_residual_ex(self._h, _i32(m), out))
         return float(out[0])
 
+    def hr_residual_ex(self, mode):
+        """(norm, sum w H^2, sum w) of the current state."""
+        out = (C.c_double * 3)()
+        _check(lib.hr_residual_ex(self._h, _i32(int(mode)), out))
+        return float(out[0]), float(out[1]), float(out[2])
+
     def hr_residual_async(self, mode, out2):
         """out2: torch float64 CUDA tensor with >= 2 elements; receives {sum w H^2, sum w}."""
         _check(lib.hr_residual_async(self._h, _i32(int(mode)), _vp(out2.data_ptr())))
+
+    def hr_step_residual_async(self, mode, out2):
+        """Residual of the current state into out2 (as hr_residual_async), then one RK4 step."""
+        _check(lib.hr_step_residual_async(self._h, _i32(int(mode)), _vp(out2.data_ptr())))
 
     def _get(self, fn, to_host):
         t = self.torch

@@ -112,7 +112,7 @@ Layout make_layout(const hr_params* p) {
   L.off_wvol = take(np * 8);
   L.off_inner_dst = take((size_t)L.n_inner * 4 + 4);
   L.off_inner_src = take((size_t)L.n_inner * 4 + 4);
-  L.nblocks = hrk_max_partials(p->n, L.ng);
+  L.nblocks = hrk_max_partials(p->n, L.ng, p->dtype);
   L.off_partials = take((size_t)L.nblocks * 16);
   L.off_result = take(64);
   L.off_counters = take(256);
@@ -388,6 +388,7 @@ hr_status hr_create(const hr_params* p, void* workspace_dev, size_t workspace_by
   s->p.punctures = s->punctures.data();
   s->stream = static_cast<cudaStream_t>(p->stream);
   s->step_graph = nullptr;
+  s->step_resid_graph[0] = s->step_resid_graph[1] = nullptr;
   s->workspace = workspace_dev;
   s->workspace_bytes = workspace_bytes;
   s->scalar_bytes = p->dtype == HR_F64 ? 8 : 4;
@@ -542,6 +543,8 @@ hr_status hr_host_setup(const hr_params* p, double* dt, double* dsmin, int64_t* 
 hr_status hr_destroy(hr_solver* s) {
   if (!s) return HR_OK;
   if (s->step_graph) cudaGraphExecDestroy(s->step_graph);
+  for (cudaGraphExec_t g : s->step_resid_graph)
+    if (g) cudaGraphExecDestroy(g);
   delete s;
   return HR_OK;
 }
@@ -556,6 +559,33 @@ hr_status hr_step(hr_solver* s, int64_t n_steps) {
       hr_status st = enqueue_rk4_step(s);
       if (st != HR_OK) return st;
     }
+  }
+  return HR_OK;
+}
+
+hr_status hr_step_residual_async(hr_solver* s, int32_t mode, double* out2_dev) {
+  if (!s || !out2_dev) return fail(HR_ERR_INVALID_ARG, "NULL argument");
+  if (mode != 0 && mode != 1) return fail(HR_ERR_INVALID_ARG, "mode must be 0 or 1");
+  double* slot = s->a.result2 + 6;  // the graph's fixed output; copied on to the caller's pointer
+  if (s->stream != nullptr && !s->step_resid_graph[mode] && !s->step_resid_tried[mode]) {
+    // captured on first use, one graph per residual mode (launch-bound on small grids)
+    s->step_resid_tried[mode] = true;
+    cudaGraph_t graph = nullptr;
+    if (cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+      const cudaError_t le = hrk_step_with_residual(s, mode, slot);
+      const cudaError_t ce = cudaStreamEndCapture(s->stream, &graph);
+      if (le == cudaSuccess && ce == cudaSuccess && graph &&
+          cudaGraphInstantiate(&s->step_resid_graph[mode], graph, 0) != cudaSuccess)
+        s->step_resid_graph[mode] = nullptr;
+      if (graph) cudaGraphDestroy(graph);
+    }
+    cudaGetLastError();  // a failed capture falls back to direct launches of the same kernels
+  }
+  if (s->step_resid_graph[mode]) {
+    HR_CUDA(cudaGraphLaunch(s->step_resid_graph[mode], s->stream));
+    HR_CUDA(cudaMemcpyAsync(out2_dev, slot, 2 * sizeof(double), cudaMemcpyDeviceToDevice, s->stream));
+  } else {
+    HR_CUDA(hrk_step_with_residual(s, mode, out2_dev));
   }
   return HR_OK;
 }
@@ -619,17 +649,24 @@ hr_status hr_relax(hr_solver* s, int64_t max_steps, int64_t check_every, double 
     return HR_OK;
   };
   while (true) {
-    HR_CUDA(hrk_residual(s, mode, dev + 2 * (k & 1)));
+    // residual k belongs to the state after k blocks.  It is reduced by the first substep of the
+    // block that follows (hr_step_residual_async: no pass of its own) -- unless no block follows.
+    if (k > 0) HR_TRY(test_block(k - 1));  // long complete: the device is busy with block k-1
+    const int64_t n = max_steps - done < check_every ? max_steps - done : check_every;
+    const bool last = met || n <= 0;
+    if (last) {
+      HR_CUDA(hrk_residual(s, mode, dev + 2 * (k & 1)));
+    } else {
+      HR_TRY(hr_step_residual_async(s, mode, dev + 2 * (k & 1)));
+    }
     HR_CUDA(cudaMemcpyAsync(pin.h + 2 * (k & 1), dev + 2 * (k & 1), 2 * sizeof(double),
                             cudaMemcpyDeviceToHost, s->stream));
     HR_CUDA(cudaEventRecord(pin.ev[k & 1], s->stream));
-    if (k > 0) HR_TRY(test_block(k - 1));  // long complete: the device is busy with block k-1
-    const int64_t n = max_steps - done < check_every ? max_steps - done : check_every;
-    if (met || n <= 0) {
+    if (last) {
       HR_TRY(test_block(k));  // the residual of the final state closes the history
       break;
     }
-    HR_TRY(hr_step(s, n));
+    if (n > 1) HR_TRY(hr_step(s, n - 1));
     done += n;
     ++k;
   }
@@ -758,20 +795,30 @@ hr_status hr_profile_step(hr_solver* s, int64_t n_steps, int32_t with_residual, 
   for (auto& e : ev) HR_CUDA(cudaEventCreate(&e));
   size_t k = 0;
   for (int64_t it = 0; it < n_steps; ++it) {
-    if (with_residual) {
+    const bool fused = with_residual && s->p.variant == 0;  // stage 1 also reduces the residual
+    if (with_residual && !fused) {
       HR_CUDA(cudaEventRecord(ev[k++], s->stream));
       HR_CUDA(hrk_residual(s, s->p.residual_mode, s->a.result2));
       HR_CUDA(cudaEventRecord(ev[k++], s->stream));
     }
     for (int stage = 1; stage <= 4; ++stage) {
       HR_CUDA(cudaEventRecord(ev[k++], s->stream));
-      HR_CUDA(hrk_substep_main(s, stage));
+      if (fused && stage == 1) {
+        HR_CUDA(hrk_fused_first(s, s->p.residual_mode));
+      } else {
+        HR_CUDA(hrk_substep_main(s, stage));
+      }
       HR_CUDA(cudaEventRecord(ev[k++], s->stream));
       if (has_fill) {
         HR_CUDA(cudaEventRecord(ev[k++], s->stream));
         HR_CUDA(hrk_substep_fill(s, stage));
         HR_CUDA(cudaEventRecord(ev[k++], s->stream));
       }
+    }
+    if (fused) {  // what is left of the residual: the final reduction pass over the item partials
+      HR_CUDA(cudaEventRecord(ev[k++], s->stream));
+      HR_CUDA(hrk_residual_final(s, s->a.result2));
+      HR_CUDA(cudaEventRecord(ev[k++], s->stream));
     }
   }
   HR_CUDA(cudaStreamSynchronize(s->stream));
@@ -783,12 +830,14 @@ hr_status hr_profile_step(hr_solver* s, int64_t n_steps, int32_t with_residual, 
     dst += ms;
     return e;
   };
+  const bool fused_r = with_residual && s->p.variant == 0;
   for (int64_t it = 0; it < n_steps; ++it) {
-    if (with_residual) { HR_CUDA(el(k, acc[5])); k += 2; }
+    if (with_residual && !fused_r) { HR_CUDA(el(k, acc[5])); k += 2; }
     for (int stage = 1; stage <= 4; ++stage) {
       HR_CUDA(el(k, acc[stage - 1])); k += 2;
       if (has_fill) { HR_CUDA(el(k, acc[4])); k += 2; }
     }
+    if (fused_r) { HR_CUDA(el(k, acc[5])); k += 2; }
   }
   for (int i = 0; i < 6; ++i) ms6[i] = acc[i] / (double)n_steps;
   return HR_OK;

@@ -117,7 +117,7 @@ struct hr_solver {
   hr_params p;
   MarchPlan plan;
   int num_sms;
-  int march_grid[6];  // persistent grid size per stage kernel (0 = eval, 1..4, 5 = residual)
+  int march_grid[7];  // persistent grid size per stage kernel (0 = eval, 1..4, 5 = residual, 6 = 1 + residual)
   // TMA descriptors of the ten stored grid functions (Y, A, B, ACC (u, v), psi, S): the TW x BY
   // box of each, and the halo-tile box of the three stencil sources Y_u, A_u, B_u
   CUtensorMap tm_box[10];
@@ -133,6 +133,8 @@ struct hr_solver {
   int max_partials;
   cudaStream_t stream;
   cudaGraphExec_t step_graph;  // one RK4 step = 4 x (fused kernel, inner fill)
+  cudaGraphExec_t step_resid_graph[2];  // the same with the residual fused into stage 1, per mode
+  bool step_resid_tried[2] = {false, false};
   int launches_per_step;
   void* workspace;
   size_t workspace_bytes;
@@ -158,8 +160,13 @@ cudaError_t hrk_unpack(const hr_solver* s, void* dst_stored, const void* src_pub
 void hrk_row_geometry(int T0, int ng, size_t scalar_bytes, int* P0, int* off0);
 // residual partial sums + final deterministic pass into out2_dev
 cudaError_t hrk_residual(const hr_solver* s, int mode, double* out2_dev);
+// one RK4 step whose first substep also reduces the residual of the state it starts from
+cudaError_t hrk_step_with_residual(const hr_solver* s, int mode, double* out2_dev);
+// its pieces, for hr_profile_step: stage 1 + residual partials; the final reduction pass
+cudaError_t hrk_fused_first(const hr_solver* s, int mode);
+cudaError_t hrk_residual_final(const hr_solver* s, double* out2_dev);
 MarchPlan hrk_make_plan(const int32_t n[3], int ng, int coord, int dtype);
 // shared-memory opt-in and persistent grid sizes of the marching kernels; before graph capture
 cudaError_t hrk_prepare(hr_solver* s);
-int hrk_max_partials(const int32_t n[3], int ng);
+int hrk_max_partials(const int32_t n[3], int ng, int dtype);
 int hrk_launches_per_substep(const hr_solver* s);

@@ -439,6 +439,7 @@ StepArgs<T> make_args(const hr_solver* s, int stage, void* ku, void* kv) {
       r.in_u = P(a.Y[0]); r.in_v = P(a.Y[1]); r.out_u = P(ku); r.out_v = P(kv);
       break;
     case 1:
+    case 6:  // stage 1 fused with the residual of its input state
       r.in_u = P(a.Y[0]); r.in_v = P(a.Y[1]); r.out_u = P(a.A[0]); r.out_v = P(a.A[1]);
       break;
     case 2:
@@ -648,10 +649,11 @@ cudaError_t prepare_march(hr_solver* s) {
   if ((e = prepare_march_stage<T, NG, 3>(s, &s->march_grid[3])) != cudaSuccess) return e;
   if ((e = prepare_march_stage<T, NG, 4>(s, &s->march_grid[4])) != cudaSuccess) return e;
   if ((e = prepare_march_stage<T, NG, 5>(s, &s->march_grid[5])) != cudaSuccess) return e;
+  if ((e = prepare_march_stage<T, NG, 6>(s, &s->march_grid[6])) != cudaSuccess) return e;
   // one chunking for all stages, balanced for the RK stage kernels (stages 2, 3 dominate)
   choose_chunks(s->plan, s->g.n2, NG, s->march_grid[2]);
   const long long items = (long long)s->plan.ntx * s->plan.nty * s->plan.nzc;
-  for (int st = 0; st < 6; ++st)
+  for (int st = 0; st < 7; ++st)
     if (s->march_grid[st] > items) s->march_grid[st] = (int)items;
   return cudaSuccess;
 }
@@ -671,7 +673,7 @@ cudaError_t prepare_march_ng(hr_solver* s) {
 
 // Tensor maps of one stage: stencil source = Y (stages 0, 1, residual), A (2, 4), B (3).
 MarchMaps make_maps(const hr_solver* s, int stage) {
-  const int in = (stage == 2 || stage == 4) ? 1 : (stage == 3 ? 2 : 0);
+  const int in = (stage == 2 || stage == 4) ? 1 : (stage == 3 ? 2 : 0);  // 0, 1, 5, 6: Y
   MarchMaps m;
   m.tile = s->tm_tile[in];
   m.st[ST_FRONT] = s->tm_box[2 * in];
@@ -707,6 +709,7 @@ cudaError_t launch_march(const hr_solver* s, int stage, void* ku, void* kv, int 
     case 2: return launch_march_stage<T, NG, 2>(s, a, ra);
     case 3: return launch_march_stage<T, NG, 3>(s, a, ra);
     case 4: return launch_march_stage<T, NG, 4>(s, a, ra);
+    case 6: return launch_march_stage<T, NG, 6>(s, a, ra);
     default: return launch_march_stage<T, NG, 5>(s, a, ra);
   }
 }
@@ -762,7 +765,7 @@ cudaError_t launch_residual(const hr_solver* s, int mode, double* out2) {
     nb = (int64_t)grid.x * grid.y * grid.z;
   } else {
     e = launch_march<T, NG>(s, 5, nullptr, nullptr, mode, a.partials);
-    nb = s->march_grid[5];
+    nb = (int64_t)s->plan.ntx * s->plan.nty * s->plan.nzc;  // one partial pair per work item
   }
   if (e != cudaSuccess) return e;
   k_residual_final<<<1, 1024, 0, s->stream>>>(a.partials, nb, out2);
@@ -778,6 +781,19 @@ cudaError_t dispatch_residual(const hr_solver* s, int mode, double* out2) {
     case 4: return launch_residual<T, 4>(s, mode, out2);
     case 5: return launch_residual<T, 5>(s, mode, out2);
     case 6: return launch_residual<T, 6>(s, mode, out2);
+  }
+  return cudaErrorInvalidValue;
+}
+
+template <typename T>
+cudaError_t dispatch_fused_first(const hr_solver* s, int mode) {
+  switch (s->g.ng) {
+    case 1: return launch_march<T, 1>(s, 6, nullptr, nullptr, mode, s->a.partials);
+    case 2: return launch_march<T, 2>(s, 6, nullptr, nullptr, mode, s->a.partials);
+    case 3: return launch_march<T, 3>(s, 6, nullptr, nullptr, mode, s->a.partials);
+    case 4: return launch_march<T, 4>(s, 6, nullptr, nullptr, mode, s->a.partials);
+    case 5: return launch_march<T, 5>(s, 6, nullptr, nullptr, mode, s->a.partials);
+    case 6: return launch_march<T, 6>(s, 6, nullptr, nullptr, mode, s->a.partials);
   }
   return cudaErrorInvalidValue;
 }
@@ -804,11 +820,13 @@ cudaError_t hrk_prepare(hr_solver* s) {
   return s->p.dtype == HR_F64 ? prepare_march_ng<double>(s) : prepare_march_ng<float>(s);
 }
 
-int hrk_max_partials(const int32_t n[3], int ng) {
+int hrk_max_partials(const int32_t n[3], int ng, int dtype) {
   (void)ng;
   const int direct = ((n[0] + RBX - 1) / RBX) * ((n[1] + RBY - 1) / RBY) * n[2];
-  const int march = 32 * 1024;  // persistent grid: resident CTAs per SM x SMs
-  return direct > march ? direct : march;
+  // marching kernels: one partial pair per work item, chunks are at least 2 planes (or all of n2)
+  const MarchPlan m = hrk_make_plan(n, ng, 0, dtype);
+  const long long march = (long long)m.ntx * m.nty * (n[2] / 2 + 1);
+  return direct > march ? direct : (int)march;
 }
 
 int hrk_launches_per_substep(const hr_solver* s) {
@@ -892,6 +910,34 @@ cudaError_t hrk_eval_rhs(const hr_solver* s, void* ku, void* kv) {
   if (e != cudaSuccess) return e;
   if (s->p.variant != 2) return cudaSuccess;
   return hrk_inner_fill(s, ku, kv);
+}
+
+// Alg. 1 l.9-16 in four launches + the final reduction pass: stage 1 also accumulates the
+// residual of the state it starts from (variant 0 only).
+cudaError_t hrk_step_with_residual(const hr_solver* s, int mode, double* out2_dev) {
+  if (s->p.variant != 0) {
+    cudaError_t e0 = hrk_residual(s, mode, out2_dev);
+    for (int stage = 1; stage <= 4 && e0 == cudaSuccess; ++stage) e0 = hrk_substep(s, stage);
+    return e0;
+  }
+  cudaError_t e = s->p.dtype == HR_F64 ? dispatch_fused_first<double>(s, mode)
+                                       : dispatch_fused_first<float>(s, mode);
+  for (int stage = 2; stage <= 4 && e == cudaSuccess; ++stage) e = hrk_substep(s, stage);
+  if (e != cudaSuccess) return e;
+  const int64_t nb = (int64_t)s->plan.ntx * s->plan.nty * s->plan.nzc;
+  k_residual_final<<<1, 1024, 0, s->stream>>>(s->a.partials, nb, out2_dev);
+  return cudaGetLastError();
+}
+
+cudaError_t hrk_fused_first(const hr_solver* s, int mode) {
+  return s->p.dtype == HR_F64 ? dispatch_fused_first<double>(s, mode)
+                              : dispatch_fused_first<float>(s, mode);
+}
+
+cudaError_t hrk_residual_final(const hr_solver* s, double* out2_dev) {
+  const int64_t nb = (int64_t)s->plan.ntx * s->plan.nty * s->plan.nzc;
+  k_residual_final<<<1, 1024, 0, s->stream>>>(s->a.partials, nb, out2_dev);
+  return cudaGetLastError();
 }
 
 cudaError_t hrk_residual(const hr_solver* s, int mode, double* out2_dev) {

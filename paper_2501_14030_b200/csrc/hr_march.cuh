@@ -222,7 +222,7 @@ enum { ST_FRONT = 0, ST_PSI = 1, ST_S = 2, ST_V = 3, ST_AU = 4, ST_AV = 5, ST_YU
 
 template <int STAGE>
 __host__ __device__ constexpr int march_nstreams() {
-  return STAGE == 5 ? 3 : (STAGE <= 1 ? 4 : (STAGE == 4 ? 6 : 8));
+  return STAGE == 5 ? 3 : ((STAGE <= 1 || STAGE == 6) ? 4 : (STAGE == 4 ? 6 : 8));
 }
 
 // Geometry shared by the kernel and the host (tensor-map boxes, shared-memory size).
@@ -245,7 +245,9 @@ __host__ __device__ constexpr size_t march_smem_bytes() {
   return 128 + (size_t)(D + 1) * (G::TILE_BYTES + march_nstreams<STAGE>() * G::BOX_BYTES);
 }
 
-// STAGE 0: k -> out (hr_eval_rhs); 1..4: RK4 stages (rk_combine); 5: residual (a5).
+// STAGE 0: k -> out (hr_eval_rhs); 1..4: RK4 stages (rk_combine); 5: residual (a5);
+// 6: RK4 stage 1 that also accumulates the residual of its input state -- the bracket of Eq. 5 at
+// the state Y is exactly H of Eq. 4, so Alg. 1 l.9-11 followed by l.12-16 needs no pass of its own.
 // TW x BY points per tile, VX points per thread along i0, D planes of look-ahead.
 template <typename T, int NG, int STAGE, int TW, int BY, int VX, int D>
 __global__ void __launch_bounds__((TW / VX) * BY,
@@ -261,6 +263,9 @@ __global__ void __launch_bounds__((TW / VX) * BY,
   constexpr int NGA = G::NGA, SWA = G::SWA;
   constexpr int NGV = (NG + VX - 1) / VX * VX;  // halo rounded to whole vectors
   constexpr int NS = march_nstreams<STAGE>();
+  constexpr int RK = STAGE == 6 ? 1 : STAGE;            // which RK combine (0 = store k)
+  constexpr bool RESID = STAGE == 5 || STAGE == 6;      // accumulate sum w H^2, sum w
+  constexpr bool ADVANCE = STAGE != 5;                  // write stage outputs and ghost images
   constexpr int RING = D + 1;
   constexpr int SLOT_BYTES = G::TILE_BYTES + NS * G::BOX_BYTES;
   constexpr int U = 2 * NG + 1;
@@ -303,6 +308,7 @@ __global__ void __launch_bounds__((TW / VX) * BY,
   // (items differ in cost: boundary tiles also write ghost images), except for the residual,
   // whose per-CTA partial sums must not depend on timing (C16: fixed reduction order).
   __shared__ int s_item;
+  __shared__ double red[2][NT / 32];
   int item = blockIdx.x;
   while (item < n_items) {
     const int chunk = item / ntiles;
@@ -359,15 +365,14 @@ __global__ void __launch_bounds__((TW / VX) * BY,
       if (j < nact) {
         const int q = i0 + j + g.T0 * i1;
         l00[j] = a.L00[q]; l11[j] = a.L11[q]; l22[j] = a.L22[q]; l0[j] = a.L0[q]; l1[j] = a.L1[q];
-        if constexpr (STAGE == 5) {
-          wq[j] = ra.mode == 0 ? ra.W[q] : 1.0;
-        } else {
+        if constexpr (RESID) wq[j] = ra.mode == 0 ? ra.W[q] : 1.0;
+        if constexpr (ADVANCE) {
           c2[j] = a.C2[q];
           inplane_images |= i0 + j < 2 * NG;
         }
       }
     }
-    if (STAGE != 5 && nact > 0) {
+    if (ADVANCE && nact > 0) {
       cB = i1 < 2 * NG ? 2 * NG - 1 - i1 : -1;
       cC = i1 >= g.n1 ? 2 * (g.n1 + NG) - 1 - i1 : -1;
       inplane_images |= (cB >= 0) || (cC >= 0);
@@ -455,21 +460,22 @@ __global__ void __launch_bounds__((TW / VX) * BY,
                           l1[j] * d1[j];
             H[j] = lap + Ss.v[j] * pow_m7(psi.v[j] + HR_W(NG)[j]);
           }
-          if constexpr (STAGE == 5) {
+          if constexpr (RESID) {
 #pragma unroll
             for (int j = 0; j < VX; ++j)
               if (j < nact) {
                 num += wq[j] * (double)H[j] * (double)H[j];
                 den += wq[j];
               }
-          } else {
+          }
+          if constexpr (ADVANCE) {
             const V vin = *reinterpret_cast<const V*>(sb + ST_V * (TW * BY) + so);
             V yu{}, yv{}, au{}, av{};
-            if constexpr (STAGE >= 2 && STAGE <= 4) {
+            if constexpr (RK >= 2 && RK <= 4) {
               au = *reinterpret_cast<const V*>(sb + ST_AU * (TW * BY) + so);
               av = *reinterpret_cast<const V*>(sb + ST_AV * (TW * BY) + so);
             }
-            if constexpr (STAGE == 2 || STAGE == 3) {
+            if constexpr (RK == 2 || RK == 3) {
               yu = *reinterpret_cast<const V*>(sb + ST_YU * (TW * BY) + so);
               yv = *reinterpret_cast<const V*>(sb + ST_YV * (TW * BY) + so);
             }
@@ -479,14 +485,14 @@ __global__ void __launch_bounds__((TW / VX) * BY,
               const T uc = HR_W(NG)[j];
               const T ku = vin.v[j] - a.eta * uc;
               const T kv = c2[j] * H[j];
-              rk_values<T, STAGE>(a.dt, ku, kv, uc, vin.v[j], yu.v[j], yv.v[j], au.v[j], av.v[j],
+              rk_values<T, RK>(a.dt, ku, kv, uc, vin.v[j], yu.v[j], yv.v[j], au.v[j], av.v[j],
                                   wu.v[j], wv.v[j], nu.v[j], nv.v[j]);
             }
             const int c = cz;
             if (nact == VX) {
               *reinterpret_cast<V*>(a.out_u + c) = wu;
               *reinterpret_cast<V*>(a.out_v + c) = wv;
-              if constexpr (STAGE >= 1 && STAGE <= 3) {
+              if constexpr (RK >= 1 && RK <= 3) {
                 *reinterpret_cast<V*>(a.acc_u + c) = nu;
                 *reinterpret_cast<V*>(a.acc_v + c) = nv;
               }
@@ -496,7 +502,7 @@ __global__ void __launch_bounds__((TW / VX) * BY,
                 if (j < nact) {
                   a.out_u[c + j] = wu.v[j];
                   a.out_v[c + j] = wv.v[j];
-                  if constexpr (STAGE >= 1 && STAGE <= 3) {
+                  if constexpr (RK >= 1 && RK <= 3) {
                     a.acc_u[c + j] = nu.v[j];
                     a.acc_v[c + j] = nv.v[j];
                   }
@@ -510,10 +516,37 @@ __global__ void __launch_bounds__((TW / VX) * BY,
 #undef HR_W
       }
     }
+    if constexpr (RESID) {
+      // one partial pair per ITEM, summed in a fixed order (thread: planes in order; then lanes,
+      // then warps), so the result does not depend on which CTA ran the item or when (C16)
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        num += __shfl_down_sync(0xffffffffu, num, o);
+        den += __shfl_down_sync(0xffffffffu, den, o);
+      }
+      if ((tid & 31) == 0) {
+        red[0][tid >> 5] = num;
+        red[1][tid >> 5] = den;
+      }
+      __syncthreads();
+      if (tid == 0) {
+        double sa = 0.0, sb = 0.0;
+#pragma unroll
+        for (int w = 0; w < NT / 32; ++w) {
+          sa += red[0][w];
+          sb += red[1][w];
+        }
+        ra.partials[2 * item] = sa;
+        ra.partials[2 * item + 1] = sb;
+      }
+      num = 0.0;
+      den = 0.0;
+    }
     if constexpr (STAGE == 5) {
+      __syncthreads();  // red is reused by the next item
       item += gridDim.x;
     } else {
-      __syncthreads();  // all threads are done with this item (and with s_item)
+      __syncthreads();  // all threads are done with this item (and with s_item, red)
       if (tid == 0) s_item = (int)gridDim.x + atomicAdd(plan.counters + 2 * STAGE, 1);
       __syncthreads();
       item = s_item;
@@ -527,29 +560,7 @@ __global__ void __launch_bounds__((TW / VX) * BY,
     }
   }
 
-  if constexpr (STAGE == 5) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-      num += __shfl_down_sync(0xffffffffu, num, o);
-      den += __shfl_down_sync(0xffffffffu, den, o);
-    }
-    __shared__ double red[2][NT / 32];
-    if ((tid & 31) == 0) {
-      red[0][tid >> 5] = num;
-      red[1][tid >> 5] = den;
-    }
-    __syncthreads();
-    if (tid == 0) {
-      double sa = 0.0, sb = 0.0;
-#pragma unroll
-      for (int w = 0; w < NT / 32; ++w) {
-        sa += red[0][w];
-        sb += red[1][w];
-      }
-      ra.partials[2 * blockIdx.x] = sa;
-      ra.partials[2 * blockIdx.x + 1] = sb;
-    }
-  } else {
+  if constexpr (ADVANCE) {
     // ---------------- outer points: radiation condition (a2, C13) + RK combine ----------------
     const int n_outer = NG * g.n1 * g.n2;
     for (int m = blockIdx.x * NT + tid; m < n_outer; m += gridDim.x * NT) {
@@ -564,7 +575,7 @@ __global__ void __launch_bounds__((TW / VX) * BY,
       const T ku = radiation_k(a.in_u, c, g.P0, r0, r1, ri);
       const T kv = radiation_k(a.in_v, c, g.P0, r0, r1, ri);
       T wu, wv;
-      rk_combine<T, STAGE>(a, c, ku, kv, uc, vc, wu, wv);
+      rk_combine<T, RK>(a, c, ku, kv, uc, vc, wu, wv);
       const int cB = i1 < 2 * NG ? 2 * NG - 1 - i1 : -1;
       const int cC = i1 >= g.n1 ? 2 * (g.n1 + NG) - 1 - i1 : -1;
       if (cB >= 0 || cC >= 0 || i2 < 2 * NG || i2 >= g.n2)

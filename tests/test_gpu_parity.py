@@ -414,3 +414,31 @@ def test_batched_independent_grids(hr):
     assert abs(r - ro) <= 1e-10 * ro
     for s in together:
         s.close()
+
+
+@pytest.mark.parametrize("name,params", [SMALL[0], SMALL[4], SMALL[5], SMALL[9]],
+                         ids=[SMALL[0][0], SMALL[4][0], SMALL[5][0], SMALL[9][0]])
+def test_step_with_fused_residual(hr, name, params):
+    """hr_step_residual_async: the residual reduced by the first RK substep equals hr_residual of the
+    state before the step (same formula and summation order; the two kernel instantiations may contract
+    FMAs differently, so equal to a few ulp, not bitwise), and the step is bit for bit the same step."""
+    import torch
+    o = Oracle(params)
+    for dtype in ("f64", "f32"):
+        a = hr.Solver(params, dtype=dtype)
+        b = hr.Solver(params, dtype=dtype)
+        u0, v0 = consistent_state(o, 11, dtype)
+        a.hr_set_state(u0, v0)
+        b.hr_set_state(u0, v0)
+        for mode in (0, 1):
+            out2 = torch.zeros(2, dtype=torch.float64, device=a.device)
+            ref3 = b.hr_residual_ex(mode)
+            a.hr_step_residual_async(mode, out2)
+            b.hr_step(1)
+            a.synchronize()
+            num, den = (float(x) for x in out2.cpu())
+            tol = 1e-13 if dtype == "f64" else 1e-6
+            assert abs(num - ref3[1]) <= tol * ref3[1] and den == ref3[2], (dtype, mode, num, ref3)
+            assert np.array_equal(a.hr_get_u(), b.hr_get_u()) and np.array_equal(a.hr_get_v(), b.hr_get_v())
+        a.close()
+        b.close()
