@@ -101,6 +101,9 @@ struct HrArrays {
 #ifndef HR_MARCH_D_F64
 #define HR_MARCH_D_F64 2
 #endif
+#ifndef HR_MARCH_D_EXTRA_LIGHT
+#define HR_MARCH_D_EXTRA_LIGHT 1
+#endif
 #ifndef HR_MARCH_D_F32
 #define HR_MARCH_D_F32 2
 #endif
