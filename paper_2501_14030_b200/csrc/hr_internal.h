@@ -112,6 +112,7 @@ struct HrArrays {
 struct MarchPlan {
   int ntx, nty;  // tiles along i0, i1
   int zc, nzc;   // planes per chunk, chunks along i2
+  int gt;        // tiles per group (whole tile rows); items are chunk-major within a group
   int* counters; // device: {next item, CTAs done} per stage kernel, zero between launches
   int sph;       // 1 = SinhSpherical inner map (theta -> pi - theta under rho -> -rho)
 };

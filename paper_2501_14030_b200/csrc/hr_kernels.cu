@@ -610,7 +610,7 @@ cudaError_t encode_box(const hr_solver* s, CUtensorMap* map, void* base, int bw,
 // neighbouring tiles in step, and priming an item's 2NG-plane window costs about one plane --
 // while 32-64 planes lose up to 30 %.  So: 8 planes, shorter (down to 2) only while the grid
 // has fewer items than CTA slots (small grids, latency regime), evened out over n2.
-static void choose_chunks(MarchPlan& m, int n2, int ng, int slots) {
+static void choose_chunks(MarchPlan& m, int n2, int ng, int slots, bool f64) {
   (void)ng;
   const char* zc_env = std::getenv("HR_TUNE_ZC");  // tuning knob: planes per chunk
   int zc = 8;
@@ -623,6 +623,18 @@ static void choose_chunks(MarchPlan& m, int n2, int ng, int slots) {
   if (zc > n2) zc = n2;
   m.nzc = (n2 + zc - 1) / zc;
   m.zc = (n2 + m.nzc - 1) / m.nzc;
+  // Tiles per group: whole tile rows, about `gt_target` tiles.  Short chunks re-read the 2NG planes
+  // two consecutive chunks of a tile share; with all tiles in one group the second read comes a
+  // whole band of the grid later and misses L2.  Groups of ~256 tiles keep it in L2: fp64
+  // (DRAM-bound stages) +3 % on config 3; fp32 (issue-bound) -2 %, so fp32 keeps one group.
+  const char* gt_env = std::getenv("HR_TUNE_GT");  // tuning knob: tiles per group (0 = all)
+  const int gt_target = gt_env ? std::atoi(gt_env) : (f64 ? 256 : 0);
+  const int ntiles = m.ntx * m.nty;
+  int rows = gt_target > 0 ? (gt_target + m.ntx - 1) / m.ntx : m.nty;
+  if (rows < 1) rows = 1;
+  if (rows > m.nty) rows = m.nty;
+  m.gt = rows * m.ntx;
+  (void)ntiles;
 }
 
 // Persistent grid of one stage's kernel: resident CTAs per SM x SMs (never more than the work).
@@ -660,7 +672,7 @@ cudaError_t prepare_march(hr_solver* s) {
   if ((e = prepare_march_stage<T, NG, 5>(s, &s->march_grid[5])) != cudaSuccess) return e;
   if ((e = prepare_march_stage<T, NG, 6>(s, &s->march_grid[6])) != cudaSuccess) return e;
   // one chunking for all stages, balanced for the RK stage kernels (stages 2, 3 dominate)
-  choose_chunks(s->plan, s->g.n2, NG, s->march_grid[2]);
+  choose_chunks(s->plan, s->g.n2, NG, s->march_grid[2], sizeof(T) == 8);
   const long long items = (long long)s->plan.ntx * s->plan.nty * s->plan.nzc;
   for (int st = 0; st < 7; ++st)
     if (s->march_grid[st] > items) s->march_grid[st] = (int)items;
@@ -820,6 +832,7 @@ MarchPlan hrk_make_plan(const int32_t n[3], int ng, int coord, int dtype) {
   m.sph = coord == HR_SINHSPHERICAL ? 1 : 0;
   m.zc = n[2];
   m.nzc = 1;
+  m.gt = m.ntx * m.nty;
   (void)ng;
   return m;
 }

@@ -311,8 +311,16 @@ __global__ void __launch_bounds__((TW / VX) * BY,
   __shared__ double red[2][NT / 32];
   int item = blockIdx.x;
   while (item < n_items) {
-    const int chunk = item / ntiles;
-    const int tile_id = item - chunk * ntiles;
+    // item -> (group of tile rows, chunk, tile in group): chunk-major inside a group of plan.gt
+    // tiles, so that neighbouring tiles of the same planes run together (halo rows meet in L2)
+    // AND the chunks of a tile follow each other closely enough for the 2NG planes their
+    // windows share to still be in L2
+    const int per_group = plan.gt * plan.nzc;
+    const int grp = item / per_group;
+    const int gt_here = min(plan.gt, ntiles - grp * plan.gt);  // the last group may be smaller
+    const int rem = item - grp * per_group;
+    const int chunk = rem / gt_here;
+    const int tile_id = grp * plan.gt + (rem - chunk * gt_here);
     const int zi = chunk * plan.zc;
     const int seg = min(plan.zc, g.n2 - zi);
     const int tx = tile_id % plan.ntx, ty = tile_id / plan.ntx;
