@@ -12,9 +12,11 @@
 //     moves (HR_MARCH_ROTATE = 1 unrolls the plane loop 2 NG + 1 times instead so the window
 //     rotates without moves; that copy of the loop no longer fits the 32 KB instruction cache
 //     and measured no faster);
-//   * CTAs are persistent over (chunk of planes, tile) work items in chunk-major order, so the
-//     CTAs resident at any time work on neighbouring tiles of the same planes (halo rows meet
-//     in L2); after its first item a CTA takes the next one from an atomic counter;
+//   * CTAs are persistent over (chunk of planes, tile) work items, chunk-major within groups of
+//     tile rows, so the CTAs resident at any time work on neighbouring tiles of the same planes
+//     (halo rows meet in L2) and the chunks of a tile follow each other while the planes their
+//     windows share are still in L2; after its first item a CTA takes the next one from an
+//     atomic counter;
 //   * the reference-metric factors depend on (i0, i1) only (reading C4), so each thread loads its
 //     six coefficients once per column and keeps them in registers;
 //   * the RK combine (a4) happens in the same thread, so k never reaches HBM, and the thread that
