@@ -8,7 +8,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libhr_b200.so")
 SOURCES = ["hr_api.cu", "hr_kernels.cu"]
-HEADERS = ["hr_internal.h", "fd_tables.cuh", os.path.join(ROOT, "include", "hr.h")]
+HEADERS = ["hr_internal.h", "fd_tables.cuh", "hr_march.cuh", os.path.join(ROOT, "include", "hr.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--fmad=true"]
 

@@ -97,6 +97,11 @@ struct HrArrays {
 #define HR_MARCH_L2_HINTS 0
 #endif
 
+// 1: fp32 with two points per thread uses the sm_100 packed fp32x2 instructions (FFMA2, FADD2).
+#ifndef HR_MARCH_F32X2
+#define HR_MARCH_F32X2 1
+#endif
+
 // Planes of asynchronous look-ahead in the marching kernels.
 #ifndef HR_MARCH_D_F64
 #define HR_MARCH_D_F64 2

@@ -11,6 +11,7 @@
 #include <cuda_runtime.h>
 
 #include <cstdlib>
+#include <type_traits>
 
 #include "fd_tables.cuh"
 #include "hr_internal.h"

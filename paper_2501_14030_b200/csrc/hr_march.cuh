@@ -38,6 +38,68 @@ struct alignas(sizeof(T) * VX) Vec {
   T v[VX];
 };
 
+// Two fp32 values in one 64-bit register pair and the sm_100 packed arithmetic on them
+// (add/sub/mul/fma.f32x2 -> FADD2 / FMUL2 / FFMA2: one issue slot for two points).  lo = point 0.
+struct F2 {
+  unsigned long long r;
+};
+__device__ __forceinline__ F2 f2_pack(float lo, float hi) {
+  F2 x;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(x.r) : "f"(lo), "f"(hi));
+  return x;
+}
+__device__ __forceinline__ void f2_unpack(F2 x, float& lo, float& hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(x.r));
+}
+__device__ __forceinline__ F2 f2_bc(float w) { return f2_pack(w, w); }
+__device__ __forceinline__ F2 f2_add(F2 a, F2 b) {
+  F2 d;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d.r) : "l"(a.r), "l"(b.r));
+  return d;
+}
+__device__ __forceinline__ F2 f2_sub(F2 a, F2 b) {
+  F2 d;
+  asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d.r) : "l"(a.r), "l"(b.r));
+  return d;
+}
+__device__ __forceinline__ F2 f2_mul(F2 a, F2 b) {
+  F2 d;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d.r) : "l"(a.r), "l"(b.r));
+  return d;
+}
+__device__ __forceinline__ F2 f2_fma(F2 a, F2 b, F2 c) {
+  F2 d;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d.r) : "l"(a.r), "l"(b.r), "l"(c.r));
+  return d;
+}
+// the RK combine of rk_values on two points at once (same formulas, same order)
+template <int RK>
+__device__ __forceinline__ void rk_values_f2(float dt, F2 ku, F2 kv, F2 in_u, F2 in_v, F2 yu, F2 yv,
+                                             F2 au, F2 av, F2& wu, F2& wv, F2& nu, F2& nv) {
+  nu = f2_bc(0.f);
+  nv = nu;
+  if constexpr (RK == 0) {
+    wu = ku;
+    wv = kv;
+  } else if constexpr (RK == 1) {
+    const F2 h = f2_bc(dt * 0.5f), s = f2_bc(dt / 6.f);
+    wu = f2_fma(h, ku, in_u);
+    wv = f2_fma(h, kv, in_v);
+    nu = f2_fma(s, ku, in_u);
+    nv = f2_fma(s, kv, in_v);
+  } else if constexpr (RK == 2 || RK == 3) {
+    const F2 h = f2_bc(RK == 2 ? dt * 0.5f : dt), s = f2_bc(dt / 3.f);
+    wu = f2_fma(h, ku, yu);
+    wv = f2_fma(h, kv, yv);
+    nu = f2_fma(s, ku, au);
+    nv = f2_fma(s, kv, av);
+  } else {
+    const F2 s = f2_bc(dt / 6.f);
+    wu = f2_fma(s, ku, au);
+    wv = f2_fma(s, kv, av);
+  }
+}
+
 // Tensor maps of one launch: the halo-tile box of the stage's u and the TW x BY box of every
 // pointwise input, indexed by ST_*.
 struct alignas(64) MarchMaps {
@@ -268,6 +330,7 @@ __global__ void __launch_bounds__((TW / VX) * BY,
   constexpr int RK = STAGE == 6 ? 1 : STAGE;            // which RK combine (0 = store k)
   constexpr bool RESID = STAGE == 5 || STAGE == 6;      // accumulate sum w H^2, sum w
   constexpr bool ADVANCE = STAGE != 5;                  // write stage outputs and ghost images
+  constexpr bool PACKED = HR_MARCH_F32X2 && sizeof(T) == 4 && VX == 2;  // FFMA2 / FADD2 path
   constexpr int RING = D + 1;
   constexpr int SLOT_BYTES = G::TILE_BYTES + NS * G::BOX_BYTES;
   constexpr int U = 2 * NG + 1;
@@ -390,14 +453,32 @@ __global__ void __launch_bounds__((TW / VX) * BY,
 
     // register window: w(k)[j] = u(i0 + j, i1, z - NG + k), k = 0..2NG, kept in p[(r + k) % U]
     // with r = (z - z_begin) % U (the plane loop is unrolled U times)
-    T p[U][VX];
+    // (packed fp32 path: one 64-bit element holds both points, so that the pair stays in an aligned
+    // register pair and FFMA2 / FADD2 take it without repacking moves)
+    using WT = typename std::conditional<PACKED, unsigned long long, T>::type;
+    constexpr int WJ = PACKED ? 1 : VX;
+    WT p[U][WJ];
     if (nact > 0) {
 #pragma unroll
       for (int k = 0; k < 2 * NG; ++k) {
-        const V t = *reinterpret_cast<const V*>(a.in_u + col + (z_begin - NG + k) * s2);
+        const T* src = a.in_u + col + (z_begin - NG + k) * s2;
+        if constexpr (PACKED) {
+          p[k + (UR == 1 ? 1 : 0)][0] = *reinterpret_cast<const unsigned long long*>(src);
+        } else {
+          const V t = *reinterpret_cast<const V*>(src);
 #pragma unroll
-        for (int j = 0; j < VX; ++j) p[k + (UR == 1 ? 1 : 0)][j] = t.v[j];
+          for (int j = 0; j < VX; ++j) p[k + (UR == 1 ? 1 : 0)][j] = t.v[j];
+        }
       }
+    }
+    [[maybe_unused]] F2 l00p{}, l11p{}, l22p{}, l0p{}, l1p{}, c2p{};
+    if constexpr (PACKED) {
+      l00p = f2_pack((float)l00[0], (float)l00[VX - 1]);
+      l11p = f2_pack((float)l11[0], (float)l11[VX - 1]);
+      l22p = f2_pack((float)l22[0], (float)l22[VX - 1]);
+      l0p = f2_pack((float)l0[0], (float)l0[VX - 1]);
+      l1p = f2_pack((float)l1[0], (float)l1[VX - 1]);
+      c2p = f2_pack((float)c2[0], (float)c2[VX - 1]);
     }
 
     const int so = ly * TW + VX * lx;                                     // in a TW x BY box
@@ -424,9 +505,11 @@ __global__ void __launch_bounds__((TW / VX) * BY,
 #pragma unroll
             for (int k = 0; k < 2 * NG; ++k)
 #pragma unroll
-              for (int j = 0; j < VX; ++j) p[k][j] = p[k + 1][j];
+              for (int j = 0; j < WJ; ++j) p[k][j] = p[k + 1][j];
           }
-          {
+          if constexpr (PACKED) {
+            HR_W(2 * NG)[0] = *reinterpret_cast<const unsigned long long*>(sb + ST_FRONT * (TW * BY) + so);
+          } else {
             const V fr = *reinterpret_cast<const V*>(sb + ST_FRONT * (TW * BY) + so);
 #pragma unroll
             for (int j = 0; j < VX; ++j) HR_W(2 * NG)[j] = fr.v[j];
@@ -438,6 +521,56 @@ __global__ void __launch_bounds__((TW / VX) * BY,
 #pragma unroll
             for (int j = 0; j < VX; ++j) e[m * VX + j] = t.v[j];
           }
+          const V psi = *reinterpret_cast<const V*>(sb + ST_PSI * (TW * BY) + so);
+          const V Ss = *reinterpret_cast<const V*>(sb + ST_S * (TW * BY) + so);
+          T H[VX];
+          [[maybe_unused]] F2 H2{}, uc2{};
+          if constexpr (PACKED) {
+            // fp32, two points per thread: the i1 and i2 stencils, the combination with the metric
+            // factors, the source term and (below) the RK combine on packed pairs; the i0 stencil
+            // stays per point (its neighbour pairs straddle the register pairs)
+            auto L2 = [](const T* q) { return F2{*reinterpret_cast<const unsigned long long*>(q)}; };
+            uc2 = F2{(unsigned long long)HR_W(NG)[0]};
+            float uc_lo, uc_hi;
+            f2_unpack(uc2, uc_lo, uc_hi);
+            float d00s[2] = {(float)F::d2(0) * uc_lo, (float)F::d2(0) * uc_hi}, d0s[2] = {0.f, 0.f};
+            F2 d11 = f2_mul(f2_bc((float)F::d2(0)), uc2), d22 = d11, d1 = f2_bc(0.f);
+#pragma unroll
+            for (int k = 1; k <= NG; ++k) {
+              const F2 up2 = L2(tl + to + k * SWA), dn2 = L2(tl + to - k * SWA);
+#pragma unroll
+              for (int j = 0; j < 2; ++j) {
+                const float a0 = (float)e[NGV + j + k], b0 = (float)e[NGV + j - k];
+                d00s[j] += (float)F::d2(k) * (a0 + b0);
+                d0s[j] += (float)F::c1(k) * (a0 - b0);
+              }
+              d11 = f2_fma(f2_bc((float)F::d2(k)), f2_add(up2, dn2), d11);
+              d22 = f2_fma(f2_bc((float)F::d2(k)),
+                           f2_add(F2{(unsigned long long)HR_W(NG + k)[0]}, F2{(unsigned long long)HR_W(NG - k)[0]}),
+                           d22);
+              d1 = f2_fma(f2_bc((float)F::c1(k)), f2_sub(up2, dn2), d1);
+            }
+            F2 lap = f2_mul(l00p, f2_pack(d00s[0], d00s[1]));
+            lap = f2_fma(l11p, d11, lap);
+            lap = f2_fma(l22p, d22, lap);
+            lap = f2_fma(l0p, f2_pack(d0s[0], d0s[1]), lap);
+            lap = f2_fma(l1p, d1, lap);
+            // (psi + u)^-7: hardware reciprocal seed per lane, Newton step and powers packed
+            const F2 x = f2_add(L2(sb + ST_PSI * (TW * BY) + so), uc2);
+            float x0, x1, r0, r1;
+            f2_unpack(x, x0, x1);
+            asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r0) : "f"(x0));
+            asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r1) : "f"(x1));
+            F2 rr = f2_pack(r0, r1);
+            const F2 nx = f2_sub(f2_bc(0.f), x);
+            rr = f2_fma(rr, f2_fma(nx, rr, f2_bc(1.f)), rr);
+            const F2 t2 = f2_mul(rr, rr), t4 = f2_mul(t2, t2);
+            H2 = f2_fma(L2(sb + ST_S * (TW * BY) + so), f2_mul(f2_mul(t4, t2), rr), lap);
+            float h0, h1;
+            f2_unpack(H2, h0, h1);
+            H[0] = (T)h0;
+            H[VX - 1] = (T)h1;
+          } else {
           T d00[VX], d11[VX], d22[VX], d0[VX], d1[VX];
 #pragma unroll
           for (int j = 0; j < VX; ++j) {
@@ -461,14 +594,12 @@ __global__ void __launch_bounds__((TW / VX) * BY,
               d1[j] += T(F::c1(k)) * (up.v[j] - dn.v[j]);
             }
           }
-          const V psi = *reinterpret_cast<const V*>(sb + ST_PSI * (TW * BY) + so);
-          const V Ss = *reinterpret_cast<const V*>(sb + ST_S * (TW * BY) + so);
-          T H[VX];
 #pragma unroll
           for (int j = 0; j < VX; ++j) {
             const T lap = l00[j] * d00[j] + l11[j] * d11[j] + l22[j] * d22[j] + l0[j] * d0[j] +
                           l1[j] * d1[j];
             H[j] = lap + Ss.v[j] * pow_m7(psi.v[j] + HR_W(NG)[j]);
+          }
           }
           if constexpr (RESID) {
 #pragma unroll
@@ -490,13 +621,43 @@ __global__ void __launch_bounds__((TW / VX) * BY,
               yv = *reinterpret_cast<const V*>(sb + ST_YV * (TW * BY) + so);
             }
             V wu, wv, nu, nv;  // stage output and the new running sum
+            if constexpr (PACKED) {
+              auto L2 = [](const T* q) { return F2{*reinterpret_cast<const unsigned long long*>(q)}; };
+              auto toV = [](F2 x) {
+                V v;
+                float lo, hi;
+                f2_unpack(x, lo, hi);
+                v.v[0] = (T)lo;
+                v.v[VX - 1] = (T)hi;
+                return v;
+              };
+              const F2 vin2 = L2(sb + ST_V * (TW * BY) + so);
+              const F2 ku = f2_fma(f2_bc(-(float)a.eta), uc2, vin2);
+              const F2 kv = f2_mul(c2p, H2);
+              F2 yu2{}, yv2{}, au2{}, av2{};
+              if constexpr (RK >= 2 && RK <= 4) {
+                au2 = L2(sb + ST_AU * (TW * BY) + so);
+                av2 = L2(sb + ST_AV * (TW * BY) + so);
+              }
+              if constexpr (RK == 2 || RK == 3) {
+                yu2 = L2(sb + ST_YU * (TW * BY) + so);
+                yv2 = L2(sb + ST_YV * (TW * BY) + so);
+              }
+              F2 wu2, wv2, nu2, nv2;
+              rk_values_f2<RK>((float)a.dt, ku, kv, uc2, vin2, yu2, yv2, au2, av2, wu2, wv2, nu2, nv2);
+              wu = toV(wu2);
+              wv = toV(wv2);
+              nu = toV(nu2);
+              nv = toV(nv2);
+            } else {
 #pragma unroll
-            for (int j = 0; j < VX; ++j) {
-              const T uc = HR_W(NG)[j];
-              const T ku = vin.v[j] - a.eta * uc;
-              const T kv = c2[j] * H[j];
-              rk_values<T, RK>(a.dt, ku, kv, uc, vin.v[j], yu.v[j], yv.v[j], au.v[j], av.v[j],
-                                  wu.v[j], wv.v[j], nu.v[j], nv.v[j]);
+              for (int j = 0; j < VX; ++j) {
+                const T uc = HR_W(NG)[j];
+                const T ku = vin.v[j] - a.eta * uc;
+                const T kv = c2[j] * H[j];
+                rk_values<T, RK>(a.dt, ku, kv, uc, vin.v[j], yu.v[j], yv.v[j], au.v[j], av.v[j],
+                                 wu.v[j], wv.v[j], nu.v[j], nv.v[j]);
+              }
             }
             const int c = cz;
             if (nact == VX) {
