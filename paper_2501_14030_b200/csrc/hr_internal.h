@@ -102,6 +102,11 @@ struct HrArrays {
 #define HR_MARCH_F32X2 1
 #endif
 
+// Copies of the plane-loop body per window shift (HR_MARCH_ROTATE = 0).
+#ifndef HR_MARCH_UNROLL
+#define HR_MARCH_UNROLL 2
+#endif
+
 // Planes of asynchronous look-ahead in the marching kernels.
 #ifndef HR_MARCH_D_F64
 #define HR_MARCH_D_F64 2

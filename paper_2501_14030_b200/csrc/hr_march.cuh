@@ -8,10 +8,12 @@
 //     compute threads spend no instructions on load addresses;
 //   * a thread owns VX consecutive points along i0 and reads / writes them as one vector
 //     (rows of the stored layout start on 128-byte lines, hr_internal.h);
-//   * the i2 stencil is a register window of 2 NG + 1 planes per point, shifted by register
-//     moves (HR_MARCH_ROTATE = 1 unrolls the plane loop 2 NG + 1 times instead so the window
-//     rotates without moves; that copy of the loop no longer fits the 32 KB instruction cache
-//     and measured no faster);
+//   * the i2 stencil is a register window of 2 NG + 1 planes per point; the plane loop is
+//     unrolled twice over a window one plane longer, which is shifted by two planes per pass
+//     (HR_MARCH_ROTATE = 1 unrolls 2 NG + 1 times instead so the window rotates without moves;
+//     that copy of the loop no longer fits the 32 KB instruction cache and measured no faster);
+//   * fp32: a thread owns two points and does the i1 / i2 stencils, the metric combination, the
+//     source term and the RK combine on packed pairs (fma/add/mul.f32x2 -> FFMA2 / FADD2 / FMUL2);
 //   * CTAs are persistent over (chunk of planes, tile) work items, chunk-major within groups of
 //     tile rows, so the CTAs resident at any time work on neighbouring tiles of the same planes
 //     (halo rows meet in L2) and the chunks of a tile follow each other while the planes their
@@ -337,7 +339,10 @@ __global__ void __launch_bounds__((TW / VX) * BY,
   // UR = U: the plane loop is unrolled U times and the i2 window rotates through the registers
   // without moves; UR = 1: one copy of the body (fits the 32 KB instruction cache) and the
   // window is shifted with register moves.
-  constexpr int UR = HR_MARCH_ROTATE ? U : 1;
+  // Otherwise the loop is unrolled HR_MARCH_UNROLL times over a window of U + UR - 1 planes that
+  // is shifted by UR planes once per unrolled block (2NG register moves per block, not per plane).
+  constexpr int UR = HR_MARCH_ROTATE ? U : HR_MARCH_UNROLL;
+  constexpr int WS = HR_MARCH_ROTATE ? U : U + UR - 1;  // window registers (planes)
   static_assert(NGA % VX == 0 && TW % VX == 0, "vector alignment");
 
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -457,17 +462,17 @@ __global__ void __launch_bounds__((TW / VX) * BY,
     // register pair and FFMA2 / FADD2 take it without repacking moves)
     using WT = typename std::conditional<PACKED, unsigned long long, T>::type;
     constexpr int WJ = PACKED ? 1 : VX;
-    WT p[U][WJ];
+    WT p[WS][WJ];
     if (nact > 0) {
 #pragma unroll
       for (int k = 0; k < 2 * NG; ++k) {
         const T* src = a.in_u + col + (z_begin - NG + k) * s2;
         if constexpr (PACKED) {
-          p[k + (UR == 1 ? 1 : 0)][0] = *reinterpret_cast<const unsigned long long*>(src);
+          p[k][0] = *reinterpret_cast<const unsigned long long*>(src);
         } else {
           const V t = *reinterpret_cast<const V*>(src);
 #pragma unroll
-          for (int j = 0; j < VX; ++j) p[k + (UR == 1 ? 1 : 0)][j] = t.v[j];
+          for (int j = 0; j < VX; ++j) p[k][j] = t.v[j];
         }
       }
     }
@@ -490,7 +495,7 @@ __global__ void __launch_bounds__((TW / VX) * BY,
       for (int r = 0; r < UR; ++r) {
         const int z = zb + r;
         if (z >= z_end) break;
-#define HR_W(k) p[(r + (k)) % U]
+#define HR_W(k) p[HR_MARCH_ROTATE ? (r + (k)) % U : r + (k)]
         __syncthreads();  // every thread is done with plane z-1: its slot can be refilled
         if (tid == 0 && z + D < z_end) issue(z + D, sl == 0 ? RING - 1 : sl - 1);  // (sl + D) % RING
         mbar_wait(bars_u32 + sl * 8, par);  // the boxes of plane z have landed
@@ -501,12 +506,6 @@ __global__ void __launch_bounds__((TW / VX) * BY,
           par ^= 1u;
         }
         if (nact > 0) {
-          if constexpr (UR == 1) {  // no rotation: shift the window by one plane
-#pragma unroll
-            for (int k = 0; k < 2 * NG; ++k)
-#pragma unroll
-              for (int j = 0; j < WJ; ++j) p[k][j] = p[k + 1][j];
-          }
           if constexpr (PACKED) {
             HR_W(2 * NG)[0] = *reinterpret_cast<const unsigned long long*>(sb + ST_FRONT * (TW * BY) + so);
           } else {
@@ -685,6 +684,12 @@ __global__ void __launch_bounds__((TW / VX) * BY,
         }
         cz += s2;
 #undef HR_W
+      }
+      if constexpr (!HR_MARCH_ROTATE) {  // shift the window by the UR planes just done
+#pragma unroll
+        for (int k = 0; k < 2 * NG; ++k)
+#pragma unroll
+          for (int j = 0; j < WJ; ++j) p[k][j] = p[k + UR][j];
       }
     }
     if constexpr (RESID) {
