@@ -118,7 +118,8 @@ HR_API hr_status hr_step(hr_solver* s, int64_t n_steps);
  * sum w } to out2_dev, device pointer) and then one RK4 step.  In the default arrangement the
  * residual costs no pass of its own: the bracket of Eq. 5 that the first RK substep evaluates at
  * the state Y is exactly H of Eq. 4, so that substep also reduces w H^2 (one partial pair per
- * work item, summed in a fixed order; equal to hr_residual_async's result to a few ulp).  Asynchronous. */
+ * work item, summed in a fixed order by the last CTA to finish; equal to hr_residual_async's result
+ * to a few ulp).  Asynchronous. */
 HR_API hr_status hr_step_residual_async(hr_solver* s, int32_t mode, double* out2_dev);
 
 /* PAPER.md:337-347 (N independent grids advanced together): n_steps RK4 steps of each of the n
@@ -203,7 +204,7 @@ HR_API hr_status hr_host_setup(const hr_params* p, double* dt, double* dsmin, in
  * { fused substep kernel of stage 1, 2, 3, 4, the four inner fills together (0 in the default
  * arrangement, whose substep kernel writes the ghost images itself), residual }.  With
  * with_residual != 0 the default arrangement runs the step as hr_step_residual_async does: stage 1
- * includes the residual accumulation and "residual" is the final reduction pass alone.
+ * includes the residual (accumulation and final reduction) and "residual" is 0.
  * Synchronises the stream. */
 HR_API hr_status hr_profile_step(hr_solver* s, int64_t n_steps, int32_t with_residual, double* ms6);
 

@@ -786,7 +786,7 @@ hr_status hr_profile_step(hr_solver* s, int64_t n_steps, int32_t with_residual, 
   if (n_steps < 1 || n_steps > 4096) return fail(HR_ERR_INVALID_ARG, "n_steps must be in 1..4096");
   // one event pair per launch; elapsed times are read after a single synchronisation at the end
   const bool has_fill = hrk_launches_per_substep(s) >= 2;  // variants 1, 2: launches after the main kernel
-  const int per_step = 4 + (has_fill ? 4 : 0) + (with_residual ? 1 : 0);
+  const int per_step = 4 + (has_fill ? 4 : 0) + (with_residual && s->p.variant != 0 ? 1 : 0);
   std::vector<cudaEvent_t> ev((size_t)n_steps * per_step * 2, nullptr);
   struct Cleanup {
     std::vector<cudaEvent_t>& ev;
@@ -804,7 +804,7 @@ hr_status hr_profile_step(hr_solver* s, int64_t n_steps, int32_t with_residual, 
     for (int stage = 1; stage <= 4; ++stage) {
       HR_CUDA(cudaEventRecord(ev[k++], s->stream));
       if (fused && stage == 1) {
-        HR_CUDA(hrk_fused_first(s, s->p.residual_mode));
+        HR_CUDA(hrk_fused_first(s, s->p.residual_mode, s->a.result2));
       } else {
         HR_CUDA(hrk_substep_main(s, stage));
       }
@@ -814,11 +814,6 @@ hr_status hr_profile_step(hr_solver* s, int64_t n_steps, int32_t with_residual, 
         HR_CUDA(hrk_substep_fill(s, stage));
         HR_CUDA(cudaEventRecord(ev[k++], s->stream));
       }
-    }
-    if (fused) {  // what is left of the residual: the final reduction pass over the item partials
-      HR_CUDA(cudaEventRecord(ev[k++], s->stream));
-      HR_CUDA(hrk_residual_final(s, s->a.result2));
-      HR_CUDA(cudaEventRecord(ev[k++], s->stream));
     }
   }
   HR_CUDA(cudaStreamSynchronize(s->stream));
@@ -837,7 +832,6 @@ hr_status hr_profile_step(hr_solver* s, int64_t n_steps, int32_t with_residual, 
       HR_CUDA(el(k, acc[stage - 1])); k += 2;
       if (has_fill) { HR_CUDA(el(k, acc[4])); k += 2; }
     }
-    if (fused_r) { HR_CUDA(el(k, acc[5])); k += 2; }
   }
   for (int i = 0; i < 6; ++i) ms6[i] = acc[i] / (double)n_steps;
   return HR_OK;

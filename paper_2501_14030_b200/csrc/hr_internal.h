@@ -176,9 +176,8 @@ void hrk_row_geometry(int T0, int ng, size_t scalar_bytes, int* P0, int* off0);
 cudaError_t hrk_residual(const hr_solver* s, int mode, double* out2_dev);
 // one RK4 step whose first substep also reduces the residual of the state it starts from
 cudaError_t hrk_step_with_residual(const hr_solver* s, int mode, double* out2_dev);
-// its pieces, for hr_profile_step: stage 1 + residual partials; the final reduction pass
-cudaError_t hrk_fused_first(const hr_solver* s, int mode);
-cudaError_t hrk_residual_final(const hr_solver* s, double* out2_dev);
+// its first launch alone (hr_profile_step): stage 1 + residual, reduced into out2_dev
+cudaError_t hrk_fused_first(const hr_solver* s, int mode, double* out2_dev);
 MarchPlan hrk_make_plan(const int32_t n[3], int ng, int coord, int dtype);
 // shared-memory opt-in and persistent grid sizes of the marching kernels; before graph capture
 cudaError_t hrk_prepare(hr_solver* s);

@@ -722,9 +722,9 @@ cudaError_t launch_march_stage(const hr_solver* s, const StepArgs<T>& a, const R
 
 template <typename T, int NG>
 cudaError_t launch_march(const hr_solver* s, int stage, void* ku, void* kv, int mode,
-                         double* partials) {
+                         double* partials, double* out2 = nullptr) {
   const StepArgs<T> a = make_args<T>(s, stage, ku, kv);
-  const ResidArgs ra{s->a.Wvol, partials, mode};
+  const ResidArgs ra{s->a.Wvol, partials, mode, out2};
   switch (stage) {
     case 0: return launch_march_stage<T, NG, 0>(s, a, ra);
     case 1: return launch_march_stage<T, NG, 1>(s, a, ra);
@@ -786,8 +786,8 @@ cudaError_t launch_residual(const hr_solver* s, int mode, double* out2) {
     e = cudaGetLastError();
     nb = (int64_t)grid.x * grid.y * grid.z;
   } else {
-    e = launch_march<T, NG>(s, 5, nullptr, nullptr, mode, a.partials);
-    nb = (int64_t)s->plan.ntx * s->plan.nty * s->plan.nzc;  // one partial pair per work item
+    // one partial pair per work item; the last CTA to finish sums them into out2
+    return launch_march<T, NG>(s, 5, nullptr, nullptr, mode, a.partials, out2);
   }
   if (e != cudaSuccess) return e;
   k_residual_final<<<1, 1024, 0, s->stream>>>(a.partials, nb, out2);
@@ -808,14 +808,14 @@ cudaError_t dispatch_residual(const hr_solver* s, int mode, double* out2) {
 }
 
 template <typename T>
-cudaError_t dispatch_fused_first(const hr_solver* s, int mode) {
+cudaError_t dispatch_fused_first(const hr_solver* s, int mode, double* out2) {
   switch (s->g.ng) {
-    case 1: return launch_march<T, 1>(s, 6, nullptr, nullptr, mode, s->a.partials);
-    case 2: return launch_march<T, 2>(s, 6, nullptr, nullptr, mode, s->a.partials);
-    case 3: return launch_march<T, 3>(s, 6, nullptr, nullptr, mode, s->a.partials);
-    case 4: return launch_march<T, 4>(s, 6, nullptr, nullptr, mode, s->a.partials);
-    case 5: return launch_march<T, 5>(s, 6, nullptr, nullptr, mode, s->a.partials);
-    case 6: return launch_march<T, 6>(s, 6, nullptr, nullptr, mode, s->a.partials);
+    case 1: return launch_march<T, 1>(s, 6, nullptr, nullptr, mode, s->a.partials, out2);
+    case 2: return launch_march<T, 2>(s, 6, nullptr, nullptr, mode, s->a.partials, out2);
+    case 3: return launch_march<T, 3>(s, 6, nullptr, nullptr, mode, s->a.partials, out2);
+    case 4: return launch_march<T, 4>(s, 6, nullptr, nullptr, mode, s->a.partials, out2);
+    case 5: return launch_march<T, 5>(s, 6, nullptr, nullptr, mode, s->a.partials, out2);
+    case 6: return launch_march<T, 6>(s, 6, nullptr, nullptr, mode, s->a.partials, out2);
   }
   return cudaErrorInvalidValue;
 }
@@ -935,32 +935,22 @@ cudaError_t hrk_eval_rhs(const hr_solver* s, void* ku, void* kv) {
   return hrk_inner_fill(s, ku, kv);
 }
 
-// Alg. 1 l.9-16 in four launches + the final reduction pass: stage 1 also accumulates the
-// residual of the state it starts from (variant 0 only).
+// Alg. 1 l.9-16 in four launches: stage 1 also accumulates the residual of the state it starts
+// from and its last CTA reduces the item partials into out2_dev (variant 0 only).
 cudaError_t hrk_step_with_residual(const hr_solver* s, int mode, double* out2_dev) {
   if (s->p.variant != 0) {
     cudaError_t e0 = hrk_residual(s, mode, out2_dev);
     for (int stage = 1; stage <= 4 && e0 == cudaSuccess; ++stage) e0 = hrk_substep(s, stage);
     return e0;
   }
-  cudaError_t e = s->p.dtype == HR_F64 ? dispatch_fused_first<double>(s, mode)
-                                       : dispatch_fused_first<float>(s, mode);
+  cudaError_t e = hrk_fused_first(s, mode, out2_dev);
   for (int stage = 2; stage <= 4 && e == cudaSuccess; ++stage) e = hrk_substep(s, stage);
-  if (e != cudaSuccess) return e;
-  const int64_t nb = (int64_t)s->plan.ntx * s->plan.nty * s->plan.nzc;
-  k_residual_final<<<1, 1024, 0, s->stream>>>(s->a.partials, nb, out2_dev);
-  return cudaGetLastError();
+  return e;
 }
 
-cudaError_t hrk_fused_first(const hr_solver* s, int mode) {
-  return s->p.dtype == HR_F64 ? dispatch_fused_first<double>(s, mode)
-                              : dispatch_fused_first<float>(s, mode);
-}
-
-cudaError_t hrk_residual_final(const hr_solver* s, double* out2_dev) {
-  const int64_t nb = (int64_t)s->plan.ntx * s->plan.nty * s->plan.nzc;
-  k_residual_final<<<1, 1024, 0, s->stream>>>(s->a.partials, nb, out2_dev);
-  return cudaGetLastError();
+cudaError_t hrk_fused_first(const hr_solver* s, int mode, double* out2_dev) {
+  return s->p.dtype == HR_F64 ? dispatch_fused_first<double>(s, mode, out2_dev)
+                              : dispatch_fused_first<float>(s, mode, out2_dev);
 }
 
 cudaError_t hrk_residual(const hr_solver* s, int mode, double* out2_dev) {

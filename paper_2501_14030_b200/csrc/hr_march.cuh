@@ -31,8 +31,9 @@
 
 struct ResidArgs {
   const double* W;   // |h0 h1 h2| plane (C16)
-  double* partials;  // 2 doubles per marching CTA
+  double* partials;  // 2 doubles per work item
   int mode;
+  double* out2;      // { sum w H^2, sum w }, written by the last CTA to finish
 };
 
 template <typename T, int VX>
@@ -728,11 +729,60 @@ __global__ void __launch_bounds__((TW / VX) * BY,
       item = s_item;
     }
   }
-  if constexpr (STAGE != 5) {
-    // the last CTA to leave the item loop re-arms the counters for the next launch of this stage
-    if (tid == 0 && atomicAdd(plan.counters + 2 * STAGE + 1, 1) == (int)gridDim.x - 1) {
-      plan.counters[2 * STAGE] = 0;
-      plan.counters[2 * STAGE + 1] = 0;
+  // The last CTA to leave the item loop re-arms the counters for the next launch of this stage
+  // and, for the residual stages, sums the item partials in a fixed order (thread t takes items
+  // t, t + NT, ...; then a fixed tree), so the reduction needs no launch of its own and its
+  // result does not depend on which CTA happens to be last (C16).
+  if constexpr (STAGE != 5 || RESID) {
+    __shared__ int s_last;
+    if (tid == 0) {
+      if constexpr (RESID) __threadfence();  // this CTA's partials before its "done" tick
+      s_last = atomicAdd(plan.counters + 2 * STAGE + 1, 1) == (int)gridDim.x - 1;
+    }
+    __syncthreads();
+    if (s_last) {
+      if constexpr (RESID) {
+        __threadfence();
+        double sa = 0.0, sb = 0.0;
+        // batches of 8 independent 16-byte loads, added in index order (latency-bound otherwise)
+        const double2* pp = reinterpret_cast<const double2*>(ra.partials);
+        int i = tid;
+        for (; i + 7 * NT < n_items; i += 8 * NT) {
+          double2 v[8];
+#pragma unroll
+          for (int q = 0; q < 8; ++q) v[q] = __ldcg(pp + i + q * NT);
+#pragma unroll
+          for (int q = 0; q < 8; ++q) {
+            sa += v[q].x;
+            sb += v[q].y;
+          }
+        }
+        for (; i < n_items; i += NT) {
+          const double2 v = __ldcg(pp + i);
+          sa += v.x;
+          sb += v.y;
+        }
+        __shared__ double fin[2][NT];
+        fin[0][tid] = sa;
+        fin[1][tid] = sb;
+        __syncthreads();
+#pragma unroll
+        for (int o = NT / 2; o > 0; o >>= 1) {
+          if (tid < o) {
+            fin[0][tid] += fin[0][tid + o];
+            fin[1][tid] += fin[1][tid + o];
+          }
+          __syncthreads();
+        }
+        if (tid == 0) {
+          ra.out2[0] = fin[0][0];
+          ra.out2[1] = fin[1][0];
+        }
+      }
+      if (tid == 0) {
+        plan.counters[2 * STAGE] = 0;
+        plan.counters[2 * STAGE + 1] = 0;
+      }
     }
   }
 
