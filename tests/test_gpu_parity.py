@@ -442,3 +442,33 @@ def test_step_with_fused_residual(hr, name, params):
             assert np.array_equal(a.hr_get_u(), b.hr_get_u()) and np.array_equal(a.hr_get_v(), b.hr_get_v())
         a.close()
         b.close()
+
+
+def test_work_item_order_knobs_do_not_change_results(hr, monkeypatch):
+    """The (group, chunk, tile) decode of the marching kernels with ragged groups and chunks: tuning
+    knobs HR_TUNE_GT / HR_TUNE_ZC change the order in which work items run, never what they compute."""
+    params = W.sweep_point(7, (70, 99, 14), "SinhSymTP", 6)
+    o = Oracle(params)
+    for dtype in ("f64", "f32"):
+        u0, v0 = consistent_state(o, 21, dtype)
+        ref = None
+        for gt, zc in ((None, None), ("7", "3"), ("10", "5"), ("1", "14")):
+            if gt is None:
+                monkeypatch.delenv("HR_TUNE_GT", raising=False)
+                monkeypatch.delenv("HR_TUNE_ZC", raising=False)
+            else:
+                monkeypatch.setenv("HR_TUNE_GT", gt)
+                monkeypatch.setenv("HR_TUNE_ZC", zc)
+            s = hr.Solver(params, dtype=dtype)
+            s.hr_set_state(u0, v0)
+            ku, kv = s.hr_eval_rhs()
+            s.hr_step(3)
+            got = (ku, kv, s.hr_get_u(), s.hr_get_v())
+            s.close()
+            if ref is None:
+                ref = got
+                oku, okv = o.rhs(u0.astype(np.float64), v0.astype(np.float64))
+                assert relmax(ku, oku) <= TOL_RHS[dtype] and relmax(kv, okv) <= TOL_RHS[dtype]
+            else:
+                for a, b in zip(got, ref):
+                    assert np.array_equal(a, b)
