@@ -65,8 +65,9 @@ struct HrArrays {
 };
 
 // Tiles of the marching arrangement (hr_march.cuh): TW x BY points, VX points per thread.
-// Measured on config 3 (profiles/r1b.md, r1c.md): 4-row tiles (128 threads, 4-5 CTAs per SM) beat
-// 8-row tiles (256 threads, 2-3 CTAs) by 3-4 % -- the per-plane barrier spans fewer warps.
+// Measured on config 3 (profiles/r1b.md, r1c.md): 4-row tiles (128 threads, 5 CTAs per SM) beat
+// 8-row tiles (256 threads, 2-3 CTAs) by 3-4 % -- the per-plane barrier spans fewer warps.  The
+// fp64 kernels fit 96 registers without spills, so 5 CTAs per SM (4: -1 %, 6: -1 %).
 #ifndef HR_TW_F64
 #define HR_TW_F64 32
 #define HR_BY_F64 4
@@ -80,7 +81,7 @@ struct HrArrays {
 
 // Minimum resident CTAs per SM the marching kernels are compiled for (register cap).
 #ifndef HR_MARCH_MINB_F64
-#define HR_MARCH_MINB_F64 4
+#define HR_MARCH_MINB_F64 5
 #endif
 #ifndef HR_MARCH_MINB_F32
 #define HR_MARCH_MINB_F32 5
