@@ -53,7 +53,7 @@ hr_status validate(const hr_params* p) {
     return fail(HR_ERR_UNSUPPORTED, "coord %d unknown", p->coord);
   if (p->dtype != HR_F64 && p->dtype != HR_F32)
     return fail(HR_ERR_UNSUPPORTED, "dtype %d unknown", p->dtype);
-  if (p->variant < 0 || p->variant > 2)
+  if (p->variant < 0 || p->variant > 3)
     return fail(HR_ERR_UNSUPPORTED, "variant %d unknown", p->variant);
   const int ng = p->fd_order / 2;
   for (int a = 0; a < 3; ++a)
@@ -786,7 +786,7 @@ hr_status hr_profile_step(hr_solver* s, int64_t n_steps, int32_t with_residual, 
   if (n_steps < 1 || n_steps > 4096) return fail(HR_ERR_INVALID_ARG, "n_steps must be in 1..4096");
   // one event pair per launch; elapsed times are read after a single synchronisation at the end
   const bool has_fill = hrk_launches_per_substep(s) >= 2;  // variants 1, 2: launches after the main kernel
-  const int per_step = 4 + (has_fill ? 4 : 0) + (with_residual && s->p.variant != 0 ? 1 : 0);
+  const int per_step = 4 + (has_fill ? 4 : 0) + (with_residual && (s->p.variant == 1 || s->p.variant == 2) ? 1 : 0);
   std::vector<cudaEvent_t> ev((size_t)n_steps * per_step * 2, nullptr);
   struct Cleanup {
     std::vector<cudaEvent_t>& ev;
@@ -795,7 +795,7 @@ hr_status hr_profile_step(hr_solver* s, int64_t n_steps, int32_t with_residual, 
   for (auto& e : ev) HR_CUDA(cudaEventCreate(&e));
   size_t k = 0;
   for (int64_t it = 0; it < n_steps; ++it) {
-    const bool fused = with_residual && s->p.variant == 0;  // stage 1 also reduces the residual
+    const bool fused = with_residual && (s->p.variant == 0 || s->p.variant == 3);  // stage 1 carries it
     if (with_residual && !fused) {
       HR_CUDA(cudaEventRecord(ev[k++], s->stream));
       HR_CUDA(hrk_residual(s, s->p.residual_mode, s->a.result2));
@@ -825,7 +825,7 @@ hr_status hr_profile_step(hr_solver* s, int64_t n_steps, int32_t with_residual, 
     dst += ms;
     return e;
   };
-  const bool fused_r = with_residual && s->p.variant == 0;
+  const bool fused_r = with_residual && (s->p.variant == 0 || s->p.variant == 3);
   for (int64_t it = 0; it < n_steps; ++it) {
     if (with_residual && !fused_r) { HR_CUDA(el(k, acc[5])); k += 2; }
     for (int stage = 1; stage <= 4; ++stage) {

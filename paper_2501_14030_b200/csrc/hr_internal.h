@@ -132,11 +132,12 @@ struct hr_solver {
   hr_params p;
   MarchPlan plan;
   int num_sms;
+  int march_grid_lean[7] = {0, 0, 0, 0, 0, 0, 0};  // variant 0: the ACC-free stages, by stage % 10
   int march_grid[7];  // persistent grid size per stage kernel (0 = eval, 1..4, 5 = residual, 6 = 1 + residual)
   // TMA descriptors of the ten stored grid functions (Y, A, B, ACC (u, v), psi, S): the TW x BY
   // box of each, and the halo-tile box of the three stencil sources Y_u, A_u, B_u
   CUtensorMap tm_box[10];
-  CUtensorMap tm_tile[3];
+  CUtensorMap tm_tile[4];
   std::vector<hr_puncture> punctures;
   HrGrid g;
   HrArrays a;

@@ -51,6 +51,8 @@ template <typename T>
 struct StepArgs {
   const T* in_u;  // stage input (stencil source)
   const T* in_v;
+  const T* b_u;  // lean stage 4 only: Y2 (buffer B); there acc_u / acc_v point at Y1 (buffer A)
+  const T* b_v;
   const T* y_u;  // Y (needed by stages 2, 3; stage 1 has in == Y)
   const T* y_v;
   T* out_u;  // stages 1-3: next stage input; stage 4: Y; eval mode: k_u
@@ -452,12 +454,29 @@ StepArgs<T> make_args(const hr_solver* s, int stage, void* ku, void* kv) {
     case 4:
       r.in_u = P(a.A[0]); r.in_v = P(a.A[1]); r.out_u = P(a.Y[0]); r.out_v = P(a.Y[1]);
       break;
+    case 11:
+    case 16:  // lean: Y -> Y1 (A)
+      r.in_u = P(a.Y[0]); r.in_v = P(a.Y[1]); r.out_u = P(a.A[0]); r.out_v = P(a.A[1]);
+      break;
+    case 12:  // lean: Y1 (A) -> Y2 (B)
+      r.in_u = P(a.A[0]); r.in_v = P(a.A[1]); r.out_u = P(a.B[0]); r.out_v = P(a.B[1]);
+      break;
+    case 13:  // lean: Y2 (B) -> Y3 (the ACC buffer)
+      r.in_u = P(a.B[0]); r.in_v = P(a.B[1]); r.out_u = P(a.ACC[0]); r.out_v = P(a.ACC[1]);
+      break;
+    case 14:  // lean: Y3 -> Y, reading Y, Y1, Y2
+      r.in_u = P(a.ACC[0]); r.in_v = P(a.ACC[1]); r.out_u = P(a.Y[0]); r.out_v = P(a.Y[1]);
+      break;
     default:  // 5, residual: the stencil source is the state
       r.in_u = P(a.Y[0]); r.in_v = P(a.Y[1]);
       break;
   }
   r.y_u = P(a.Y[0]); r.y_v = P(a.Y[1]);
   r.acc_u = P(a.ACC[0]); r.acc_v = P(a.ACC[1]);
+  r.b_u = P(a.B[0]); r.b_v = P(a.B[1]);
+  if (stage == 14) {  // Y1 rides in the acc slots
+    r.acc_u = P(a.A[0]); r.acc_v = P(a.A[1]);
+  }
   r.psi = P(a.psi); r.S = P(a.S);
   r.L00 = P(a.L00); r.L11 = P(a.L11); r.L22 = P(a.L22); r.L0 = P(a.L0); r.L1 = P(a.L1);
   r.C2 = P(a.C2); r.RAD0 = P(a.RAD0); r.RAD1 = P(a.RAD1); r.RADI = P(a.RADI);
@@ -548,7 +567,7 @@ cudaError_t dispatch_paper(const hr_solver* s, int what, int stage, void* ku, vo
   return cudaErrorInvalidValue;
 }
 
-// ---- marching arrangement (variant 0) ----
+// ---- marching arrangement (variant 0: ACC-free RK4; variant 3: running-sum RK4) ----
 // Tile shape per dtype: TW x BY points, VX points per thread (16-byte vectors along i0 are
 // double2 / float4; fp64 keeps one point per thread for register room), D planes of look-ahead.
 template <typename T>
@@ -663,7 +682,7 @@ cudaError_t prepare_march(hr_solver* s) {
   void* fields[10] = {a.Y[0], a.Y[1], a.A[0], a.A[1], a.B[0], a.B[1], a.ACC[0], a.ACC[1], a.psi, a.S};
   for (int f = 0; f < 10; ++f)
     if ((e = encode_box(s, &s->tm_box[f], fields[f], C::TW, C::BY)) != cudaSuccess) return e;
-  for (int f = 0; f < 3; ++f)
+  for (int f = 0; f < 4; ++f)  // stencil sources: Y_u, A_u, B_u and (lean stage 4) ACC_u
     if ((e = encode_box(s, &s->tm_tile[f], fields[2 * f], G::SWA, G::SH)) != cudaSuccess) return e;
   if ((e = prepare_march_stage<T, NG, 0>(s, &s->march_grid[0])) != cudaSuccess) return e;
   if ((e = prepare_march_stage<T, NG, 1>(s, &s->march_grid[1])) != cudaSuccess) return e;
@@ -672,11 +691,20 @@ cudaError_t prepare_march(hr_solver* s) {
   if ((e = prepare_march_stage<T, NG, 4>(s, &s->march_grid[4])) != cudaSuccess) return e;
   if ((e = prepare_march_stage<T, NG, 5>(s, &s->march_grid[5])) != cudaSuccess) return e;
   if ((e = prepare_march_stage<T, NG, 6>(s, &s->march_grid[6])) != cudaSuccess) return e;
+  if (s->p.variant == 0) {  // the ACC-free arrangement's kernels, grid sizes indexed by stage % 10
+    if ((e = prepare_march_stage<T, NG, 11>(s, &s->march_grid_lean[1])) != cudaSuccess) return e;
+    if ((e = prepare_march_stage<T, NG, 12>(s, &s->march_grid_lean[2])) != cudaSuccess) return e;
+    if ((e = prepare_march_stage<T, NG, 13>(s, &s->march_grid_lean[3])) != cudaSuccess) return e;
+    if ((e = prepare_march_stage<T, NG, 14>(s, &s->march_grid_lean[4])) != cudaSuccess) return e;
+    if ((e = prepare_march_stage<T, NG, 16>(s, &s->march_grid_lean[6])) != cudaSuccess) return e;
+  }
   // one chunking for all stages, balanced for the RK stage kernels (stages 2, 3 dominate)
   choose_chunks(s->plan, s->g.n2, NG, s->march_grid[2], sizeof(T) == 8);
   const long long items = (long long)s->plan.ntx * s->plan.nty * s->plan.nzc;
-  for (int st = 0; st < 7; ++st)
+  for (int st = 0; st < 7; ++st) {
     if (s->march_grid[st] > items) s->march_grid[st] = (int)items;
+    if (s->march_grid_lean[st] > items) s->march_grid_lean[st] = (int)items;
+  }
   return cudaSuccess;
 }
 
@@ -695,8 +723,23 @@ cudaError_t prepare_march_ng(hr_solver* s) {
 
 // Tensor maps of one stage: stencil source = Y (stages 0, 1, residual), A (2, 4), B (3).
 MarchMaps make_maps(const hr_solver* s, int stage) {
-  const int in = (stage == 2 || stage == 4) ? 1 : (stage == 3 ? 2 : 0);  // 0, 1, 5, 6: Y
   MarchMaps m;
+  if (stage >= 10) {  // lean: front psi S v | Y | Y1 (A) | Y2 (B); sources Y, A, B, ACC
+    const int in = stage == 12 ? 1 : (stage == 13 ? 2 : (stage == 14 ? 3 : 0));
+    m.tile = s->tm_tile[in];
+    m.st[0] = s->tm_box[2 * in];
+    m.st[1] = s->tm_box[8];
+    m.st[2] = s->tm_box[9];
+    m.st[3] = s->tm_box[2 * in + 1];
+    m.st[4] = s->tm_box[0];
+    m.st[5] = s->tm_box[1];
+    m.st[6] = s->tm_box[2];
+    m.st[7] = s->tm_box[3];
+    m.st[8] = s->tm_box[4];
+    m.st[9] = s->tm_box[5];
+    return m;
+  }
+  const int in = (stage == 2 || stage == 4) ? 1 : (stage == 3 ? 2 : 0);  // 0, 1, 5, 6: Y
   m.tile = s->tm_tile[in];
   m.st[ST_FRONT] = s->tm_box[2 * in];
   m.st[ST_V] = s->tm_box[2 * in + 1];
@@ -706,6 +749,8 @@ MarchMaps make_maps(const hr_solver* s, int stage) {
   m.st[ST_AV] = s->tm_box[7];
   m.st[ST_YU] = s->tm_box[0];
   m.st[ST_YV] = s->tm_box[1];
+  m.st[8] = s->tm_box[0];
+  m.st[9] = s->tm_box[0];
   return m;
 }
 
@@ -714,7 +759,7 @@ cudaError_t launch_march_stage(const hr_solver* s, const StepArgs<T>& a, const R
   using C = MarchCfg<T>;
   constexpr size_t smem = HR_MARCH_SMEM(T, NG, STAGE);
   const dim3 block(C::TW / C::VX, C::BY, 1);
-  const dim3 grid(s->march_grid[STAGE], 1, 1);
+  const dim3 grid(STAGE >= 10 ? s->march_grid_lean[STAGE % 10] : s->march_grid[STAGE], 1, 1);
   const MarchMaps mm = make_maps(s, STAGE);
   HR_MARCH_KERNEL(T, NG, STAGE)<<<grid, block, smem, s->stream>>>(s->g, a, s->plan, ra, mm);
   return cudaGetLastError();
@@ -732,6 +777,11 @@ cudaError_t launch_march(const hr_solver* s, int stage, void* ku, void* kv, int 
     case 3: return launch_march_stage<T, NG, 3>(s, a, ra);
     case 4: return launch_march_stage<T, NG, 4>(s, a, ra);
     case 6: return launch_march_stage<T, NG, 6>(s, a, ra);
+    case 11: return launch_march_stage<T, NG, 11>(s, a, ra);
+    case 12: return launch_march_stage<T, NG, 12>(s, a, ra);
+    case 13: return launch_march_stage<T, NG, 13>(s, a, ra);
+    case 14: return launch_march_stage<T, NG, 14>(s, a, ra);
+    case 16: return launch_march_stage<T, NG, 16>(s, a, ra);
     default: return launch_march_stage<T, NG, 5>(s, a, ra);
   }
 }
@@ -749,6 +799,7 @@ cudaError_t dispatch_substep(const hr_solver* s, int stage, void* ku, void* kv) 
     }
     return cudaErrorInvalidValue;
   }
+  if (s->p.variant == 0 && stage >= 1 && stage <= 4) stage += 10;  // the ACC-free arrangement
   switch (s->g.ng) {
     case 1: return launch_march<T, 1>(s, stage, ku, kv, 0, nullptr);
     case 2: return launch_march<T, 2>(s, stage, ku, kv, 0, nullptr);
@@ -776,7 +827,7 @@ cudaError_t launch_residual(const hr_solver* s, int mode, double* out2) {
   const HrArrays& a = s->a;
   int64_t nb;
   cudaError_t e;
-  if (s->p.variant != 0) {
+  if (s->p.variant == 1 || s->p.variant == 2) {
     auto P = [](void* p) { return static_cast<const T*>(p); };
     const dim3 block(RBX, RBY, 1);
     const dim3 grid((g.n0 + RBX - 1) / RBX, (g.n1 + RBY - 1) / RBY, g.n2);
@@ -809,13 +860,14 @@ cudaError_t dispatch_residual(const hr_solver* s, int mode, double* out2) {
 
 template <typename T>
 cudaError_t dispatch_fused_first(const hr_solver* s, int mode, double* out2) {
+  const int st = s->p.variant == 0 ? 16 : 6;
   switch (s->g.ng) {
-    case 1: return launch_march<T, 1>(s, 6, nullptr, nullptr, mode, s->a.partials, out2);
-    case 2: return launch_march<T, 2>(s, 6, nullptr, nullptr, mode, s->a.partials, out2);
-    case 3: return launch_march<T, 3>(s, 6, nullptr, nullptr, mode, s->a.partials, out2);
-    case 4: return launch_march<T, 4>(s, 6, nullptr, nullptr, mode, s->a.partials, out2);
-    case 5: return launch_march<T, 5>(s, 6, nullptr, nullptr, mode, s->a.partials, out2);
-    case 6: return launch_march<T, 6>(s, 6, nullptr, nullptr, mode, s->a.partials, out2);
+    case 1: return launch_march<T, 1>(s, st, nullptr, nullptr, mode, s->a.partials, out2);
+    case 2: return launch_march<T, 2>(s, st, nullptr, nullptr, mode, s->a.partials, out2);
+    case 3: return launch_march<T, 3>(s, st, nullptr, nullptr, mode, s->a.partials, out2);
+    case 4: return launch_march<T, 4>(s, st, nullptr, nullptr, mode, s->a.partials, out2);
+    case 5: return launch_march<T, 5>(s, st, nullptr, nullptr, mode, s->a.partials, out2);
+    case 6: return launch_march<T, 6>(s, st, nullptr, nullptr, mode, s->a.partials, out2);
   }
   return cudaErrorInvalidValue;
 }
@@ -839,7 +891,7 @@ MarchPlan hrk_make_plan(const int32_t n[3], int ng, int coord, int dtype) {
 }
 
 cudaError_t hrk_prepare(hr_solver* s) {
-  if (s->p.variant != 0) return cudaSuccess;
+  if (s->p.variant == 1 || s->p.variant == 2) return cudaSuccess;
   return s->p.dtype == HR_F64 ? prepare_march_ng<double>(s) : prepare_march_ng<float>(s);
 }
 
@@ -938,7 +990,7 @@ cudaError_t hrk_eval_rhs(const hr_solver* s, void* ku, void* kv) {
 // Alg. 1 l.9-16 in four launches: stage 1 also accumulates the residual of the state it starts
 // from and its last CTA reduces the item partials into out2_dev (variant 0 only).
 cudaError_t hrk_step_with_residual(const hr_solver* s, int mode, double* out2_dev) {
-  if (s->p.variant != 0) {
+  if (s->p.variant == 1 || s->p.variant == 2) {
     cudaError_t e0 = hrk_residual(s, mode, out2_dev);
     for (int stage = 1; stage <= 4 && e0 == cudaSuccess; ++stage) e0 = hrk_substep(s, stage);
     return e0;

@@ -335,11 +335,12 @@ def test_largest_sweep_point_sampled(hr):
     s.close()
 
 
-@pytest.mark.parametrize("variant", [1, 2], ids=["paper_arrangement", "direct_fused"])
+@pytest.mark.parametrize("variant", [1, 2, 3], ids=["paper_arrangement", "direct_fused", "running_sum_rk4"])
 @pytest.mark.parametrize("name,params", [SMALL[0], SMALL[3], SMALL[5]], ids=[SMALL[0][0], SMALL[3][0], SMALL[5][0]])
 def test_other_arrangements_match_oracle(hr, name, params, variant):
-    """The comparison arrangements (variant 1: the paper's RHS -> BC -> RK kernels with k in HBM,
-    SURVEY.md f4; variant 2: round-1a direct-load fused kernel) meet the same bars as the default."""
+    """The other arrangements (variant 1: the paper's RHS -> BC -> RK kernels with k in HBM, SURVEY.md f4;
+    variant 2: round-1a direct-load fused kernel; variant 3: the marching kernels with RK4 as a running
+    sum, the default's predecessor) meet the same bars as the default."""
     o = Oracle(params)
     for dtype in ("f64", "f32"):
         s = hr.Solver(params, dtype=dtype, variant=variant)
