@@ -21,7 +21,9 @@
 //     atomic counter;
 //   * the reference-metric factors depend on (i0, i1) only (reading C4), so each thread loads its
 //     six coefficients once per column and keeps them in registers;
-//   * the RK combine (a4) happens in the same thread, so k never reaches HBM, and the thread that
+//   * the RK combine (a4) happens in the same thread, so k never reaches HBM (default: classic RK4
+//     without a running sum, STAGE codes 11-14 and 16, 34w bytes per point and step; STAGE 1-4
+//     and 6: the running-sum form, variant 3, 40w), and the thread that
 //     produces a point also writes that point's inner-ghost images (a3, reading C14/C15) --
 //     closed-form integer arithmetic, the inverse of the host's inner map -- so a substep is
 //     one launch;
