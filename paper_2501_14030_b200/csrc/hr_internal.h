@@ -115,6 +115,9 @@ struct HrArrays {
 #ifndef HR_MARCH_D_EXTRA_LIGHT
 #define HR_MARCH_D_EXTRA_LIGHT 1
 #endif
+#ifndef HR_MARCH_D_LESS_HEAVY
+#define HR_MARCH_D_LESS_HEAVY 0
+#endif
 #ifndef HR_MARCH_D_F32
 #define HR_MARCH_D_F32 2
 #endif

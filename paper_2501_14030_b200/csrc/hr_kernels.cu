@@ -586,8 +586,9 @@ struct MarchCfg<float> {
 // do not (measured on config 3).
 template <typename T, int STAGE>
 constexpr int march_depth() {
-  return MarchCfg<T>::D +
-         ((STAGE == 2 || STAGE == 3 || sizeof(T) != 8) ? 0 : HR_MARCH_D_EXTRA_LIGHT);
+  // (the 12 w kernels: stages 2, 3 of the running-sum form, stage 4 = code 14 of the ACC-free form)
+  return MarchCfg<T>::D - ((STAGE == 14 && sizeof(T) == 8) ? HR_MARCH_D_LESS_HEAVY : 0) +
+         ((STAGE == 2 || STAGE == 3 || STAGE == 14 || sizeof(T) != 8) ? 0 : HR_MARCH_D_EXTRA_LIGHT);
 }
 
 #define HR_MARCH_KERNEL(T, NG, STAGE) \
