@@ -292,12 +292,12 @@ def roofline(s, prof_ms, peak, peak_src):
     """Fused substep kernel.  `achieved` follows SURVEY.md section 8(d): 10 w algorithmic bytes per interior
     point-substep (8w, 12w, 12w, 8w for the stages of a running-sum RK4) x N_int points
     per launch / mean launch duration.  The default arrangement forms the same RK4 step without the running
-    sum and moves 8.5 w per point-substep (6w, 8w, 8w, 12w); `moved_model_*` restates the fraction with
+    sum and moves 8 w per point-substep (6w, 10w, 8w, 8w); `moved_model_*` restates the fraction with
     that count, `traffic` is the measured DRAM bytes per launch (ncu), so nothing hides behind the definition."""
     w = 8 if s.dtype == "f64" else 4
     mean_ms = sum(prof_ms[:4]) / 4.0
     bytes_per_launch = 10 * w * s.n_int
-    moved = 8.5 * w * s.n_int
+    moved = 8.0 * w * s.n_int
     achieved = bytes_per_launch / (mean_ms * 1e-3) / 1e9
     return {"bound": "hbm", "kernel": "fused substep k_march (RHS + radiation + RK combine + ghost images; stage 1 also "
                                       "reduces the residual), mean of the 4 stages",

@@ -83,9 +83,10 @@ typedef struct {
   int32_t device;        /* CUDA device ordinal                                               */
   int32_t variant;       /* kernel arrangement: 0 = default (fused RHS + radiation + RK combine +
                             ghost images in one TMA-fed marching kernel per substep; classic RK4
-                            in its ACC-free form: the stage buffers hold Y + dt/2 k1, Y + dt/2 k2,
-                            Y + dt k3 and stage 4 forms (1/3)(-Y + Y1 + 2 Y2 + Y3) + dt/6 k4, which
-                            moves 34 w instead of 40 w bytes per point and step);
+                            without a running sum: with Y1 = Y + dt/2 k1, Y2 = Y + dt/2 k2,
+                            Y3 = Y + dt k3, stage 2 also stores Q = (Y1 - Y) + 2 Y2 and stage 4
+                            forms (1/3)(Q + Y3) + dt/6 k4, which moves 32 w instead of 40 w bytes
+                            per point and step);
                             3 = the same kernels with RK4 as a running sum (ACC = Y + dt/6 k1 +
                             dt/3 k2 + dt/3 k3), the arrangement of profiles/r1b-r1f;
                             2 = direct-load fused kernel (one thread per point, stencil through

@@ -115,9 +115,6 @@ struct HrArrays {
 #ifndef HR_MARCH_D_EXTRA_LIGHT
 #define HR_MARCH_D_EXTRA_LIGHT 1
 #endif
-#ifndef HR_MARCH_D_LESS_HEAVY
-#define HR_MARCH_D_LESS_HEAVY 0
-#endif
 #ifndef HR_MARCH_D_F32
 #define HR_MARCH_D_F32 2
 #endif
@@ -140,7 +137,7 @@ struct hr_solver {
   // TMA descriptors of the ten stored grid functions (Y, A, B, ACC (u, v), psi, S): the TW x BY
   // box of each, and the halo-tile box of the three stencil sources Y_u, A_u, B_u
   CUtensorMap tm_box[10];
-  CUtensorMap tm_tile[4];
+  CUtensorMap tm_tile[3];
   std::vector<hr_puncture> punctures;
   HrGrid g;
   HrArrays a;

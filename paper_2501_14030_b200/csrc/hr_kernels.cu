@@ -51,8 +51,6 @@ template <typename T>
 struct StepArgs {
   const T* in_u;  // stage input (stencil source)
   const T* in_v;
-  const T* b_u;  // lean stage 4 only: Y2 (buffer B); there acc_u / acc_v point at Y1 (buffer A)
-  const T* b_v;
   const T* y_u;  // Y (needed by stages 2, 3; stage 1 has in == Y)
   const T* y_v;
   T* out_u;  // stages 1-3: next stage input; stage 4: Y; eval mode: k_u
@@ -461,11 +459,11 @@ StepArgs<T> make_args(const hr_solver* s, int stage, void* ku, void* kv) {
     case 12:  // lean: Y1 (A) -> Y2 (B)
       r.in_u = P(a.A[0]); r.in_v = P(a.A[1]); r.out_u = P(a.B[0]); r.out_v = P(a.B[1]);
       break;
-    case 13:  // lean: Y2 (B) -> Y3 (the ACC buffer)
-      r.in_u = P(a.B[0]); r.in_v = P(a.B[1]); r.out_u = P(a.ACC[0]); r.out_v = P(a.ACC[1]);
+    case 13:  // lean: Y2 (B) -> Y3 (A again: Y1 is no longer needed)
+      r.in_u = P(a.B[0]); r.in_v = P(a.B[1]); r.out_u = P(a.A[0]); r.out_v = P(a.A[1]);
       break;
-    case 14:  // lean: Y3 -> Y, reading Y, Y1, Y2
-      r.in_u = P(a.ACC[0]); r.in_v = P(a.ACC[1]); r.out_u = P(a.Y[0]); r.out_v = P(a.Y[1]);
+    case 14:  // lean: Y3 (A) -> Y, reading Q (the ACC buffer)
+      r.in_u = P(a.A[0]); r.in_v = P(a.A[1]); r.out_u = P(a.Y[0]); r.out_v = P(a.Y[1]);
       break;
     default:  // 5, residual: the stencil source is the state
       r.in_u = P(a.Y[0]); r.in_v = P(a.Y[1]);
@@ -473,9 +471,8 @@ StepArgs<T> make_args(const hr_solver* s, int stage, void* ku, void* kv) {
   }
   r.y_u = P(a.Y[0]); r.y_v = P(a.Y[1]);
   r.acc_u = P(a.ACC[0]); r.acc_v = P(a.ACC[1]);
-  r.b_u = P(a.B[0]); r.b_v = P(a.B[1]);
-  if (stage == 14) {  // Y1 rides in the acc slots
-    r.acc_u = P(a.A[0]); r.acc_v = P(a.A[1]);
+  if (stage == 14) {  // Q rides in the Y slots
+    r.y_u = P(a.ACC[0]); r.y_v = P(a.ACC[1]);
   }
   r.psi = P(a.psi); r.S = P(a.S);
   r.L00 = P(a.L00); r.L11 = P(a.L11); r.L22 = P(a.L22); r.L0 = P(a.L0); r.L1 = P(a.L1);
@@ -586,9 +583,10 @@ struct MarchCfg<float> {
 // do not (measured on config 3).
 template <typename T, int STAGE>
 constexpr int march_depth() {
-  // (the 12 w kernels: stages 2, 3 of the running-sum form, stage 4 = code 14 of the ACC-free form)
-  return MarchCfg<T>::D - ((STAGE == 14 && sizeof(T) == 8) ? HR_MARCH_D_LESS_HEAVY : 0) +
-         ((STAGE == 2 || STAGE == 3 || STAGE == 14 || sizeof(T) != 8) ? 0 : HR_MARCH_D_EXTRA_LIGHT);
+  // (the heavy kernels: stages 2, 3 of the running-sum form, 12 w; stage 2 = code 12 of the
+  // ACC-free form, 10 w)
+  return MarchCfg<T>::D +
+         ((STAGE == 2 || STAGE == 3 || STAGE == 12 || sizeof(T) != 8) ? 0 : HR_MARCH_D_EXTRA_LIGHT);
 }
 
 #define HR_MARCH_KERNEL(T, NG, STAGE) \
@@ -683,7 +681,7 @@ cudaError_t prepare_march(hr_solver* s) {
   void* fields[10] = {a.Y[0], a.Y[1], a.A[0], a.A[1], a.B[0], a.B[1], a.ACC[0], a.ACC[1], a.psi, a.S};
   for (int f = 0; f < 10; ++f)
     if ((e = encode_box(s, &s->tm_box[f], fields[f], C::TW, C::BY)) != cudaSuccess) return e;
-  for (int f = 0; f < 4; ++f)  // stencil sources: Y_u, A_u, B_u and (lean stage 4) ACC_u
+  for (int f = 0; f < 3; ++f)  // stencil sources: Y_u, A_u, B_u
     if ((e = encode_box(s, &s->tm_tile[f], fields[2 * f], G::SWA, G::SH)) != cudaSuccess) return e;
   if ((e = prepare_march_stage<T, NG, 0>(s, &s->march_grid[0])) != cudaSuccess) return e;
   if ((e = prepare_march_stage<T, NG, 1>(s, &s->march_grid[1])) != cudaSuccess) return e;
@@ -725,19 +723,18 @@ cudaError_t prepare_march_ng(hr_solver* s) {
 // Tensor maps of one stage: stencil source = Y (stages 0, 1, residual), A (2, 4), B (3).
 MarchMaps make_maps(const hr_solver* s, int stage) {
   MarchMaps m;
-  if (stage >= 10) {  // lean: front psi S v | Y | Y1 (A) | Y2 (B); sources Y, A, B, ACC
-    const int in = stage == 12 ? 1 : (stage == 13 ? 2 : (stage == 14 ? 3 : 0));
+  if (stage >= 10) {  // lean: front psi S v | Y (stages 2, 3) or Q = ACC (stage 4); sources Y, A, B, A
+    const int in = (stage == 12 || stage == 14) ? 1 : (stage == 13 ? 2 : 0);
+    const int ys = stage == 14 ? 6 : 0;
     m.tile = s->tm_tile[in];
     m.st[0] = s->tm_box[2 * in];
     m.st[1] = s->tm_box[8];
     m.st[2] = s->tm_box[9];
     m.st[3] = s->tm_box[2 * in + 1];
-    m.st[4] = s->tm_box[0];
-    m.st[5] = s->tm_box[1];
-    m.st[6] = s->tm_box[2];
-    m.st[7] = s->tm_box[3];
-    m.st[8] = s->tm_box[4];
-    m.st[9] = s->tm_box[5];
+    m.st[4] = s->tm_box[ys];
+    m.st[5] = s->tm_box[ys + 1];
+    m.st[6] = s->tm_box[0];
+    m.st[7] = s->tm_box[0];
     return m;
   }
   const int in = (stage == 2 || stage == 4) ? 1 : (stage == 3 ? 2 : 0);  // 0, 1, 5, 6: Y
@@ -750,8 +747,6 @@ MarchMaps make_maps(const hr_solver* s, int stage) {
   m.st[ST_AV] = s->tm_box[7];
   m.st[ST_YU] = s->tm_box[0];
   m.st[ST_YV] = s->tm_box[1];
-  m.st[8] = s->tm_box[0];
-  m.st[9] = s->tm_box[0];
   return m;
 }
 

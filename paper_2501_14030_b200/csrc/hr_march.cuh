@@ -22,7 +22,7 @@
 //   * the reference-metric factors depend on (i0, i1) only (reading C4), so each thread loads its
 //     six coefficients once per column and keeps them in registers;
 //   * the RK combine (a4) happens in the same thread, so k never reaches HBM (default: classic RK4
-//     without a running sum, STAGE codes 11-14 and 16, 34w bytes per point and step; STAGE 1-4
+//     without a running sum, STAGE codes 11-14 and 16, 32w bytes per point and step; STAGE 1-4
 //     and 6: the running-sum form, variant 3, 40w), and the thread that
 //     produces a point also writes that point's inner-ghost images (a3, reading C14/C15) --
 //     closed-form integer arithmetic, the inverse of the host's inner map -- so a substep is
@@ -106,31 +106,29 @@ __device__ __forceinline__ void rk_values_f2(float dt, F2 ku, F2 kv, F2 in_u, F2
 }
 
 // The ACC-free arrangement (k_march, STAGE >= 10), one field at a time: `in` is the stage's own
-// input (Y, Y1, Y2 or Y3), y / y1 / y2 the older buffers stage 4 needs.
+// input (Y, Y1, Y2 or Y3); y is Y for stages 2 and 3 and Q = (Y1 - Y) + 2 Y2 for stage 4.
 template <typename T, int RK>
-__device__ __forceinline__ T rk_lean(T dt, T k, T in, T y, T y1, T y2) {
+__device__ __forceinline__ T rk_lean(T dt, T k, T in, T y) {
   if constexpr (RK == 0) return k;
   if constexpr (RK == 1) return in + dt * T(0.5) * k;
   if constexpr (RK == 2) return y + dt * T(0.5) * k;
   if constexpr (RK == 3) return y + dt * k;
-  // Y_new = (1/3) (-Y + Y1 + 2 Y2 + Y3) + dt/6 k4
-  return (T(1) / T(3)) * ((y1 - y) + (T(2) * y2 + in)) + dt / T(6) * k;
+  return (T(1) / T(3)) * (y + in) + dt / T(6) * k;  // Y_new = (1/3)(Q + Y3) + dt/6 k4
 }
 template <int RK>
-__device__ __forceinline__ F2 rk_lean_f2(float dt, F2 k, F2 in, F2 y, F2 y1, F2 y2) {
+__device__ __forceinline__ F2 rk_lean_f2(float dt, F2 k, F2 in, F2 y) {
   if constexpr (RK == 0) return k;
   if constexpr (RK == 1) return f2_fma(f2_bc(dt * 0.5f), k, in);
   if constexpr (RK == 2) return f2_fma(f2_bc(dt * 0.5f), k, y);
   if constexpr (RK == 3) return f2_fma(f2_bc(dt), k, y);
-  const F2 t = f2_add(f2_sub(y1, y), f2_fma(f2_bc(2.f), y2, in));
-  return f2_fma(f2_bc(dt / 6.f), k, f2_mul(f2_bc(1.f / 3.f), t));
+  return f2_fma(f2_bc(dt / 6.f), k, f2_mul(f2_bc(1.f / 3.f), f2_add(y, in)));
 }
 
 // Tensor maps of one launch: the halo-tile box of the stage's u and the TW x BY box of every
 // pointwise input, indexed by ST_*.
 struct alignas(64) MarchMaps {
   CUtensorMap tile;
-  CUtensorMap st[10];
+  CUtensorMap st[8];
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
@@ -312,8 +310,8 @@ enum { ST_FRONT = 0, ST_PSI = 1, ST_S = 2, ST_V = 3, ST_AU = 4, ST_AV = 5, ST_YU
 
 template <int STAGE>
 __host__ __device__ constexpr int march_nstreams() {
-  if (STAGE >= 10) {  // lean (ACC-free) stages 11..14, 16: front psi S v | Y | Y1 (A) | Y2 (B)
-    return (STAGE == 11 || STAGE == 16) ? 4 : (STAGE == 14 ? 10 : 6);
+  if (STAGE >= 10) {  // ACC-free stages 11..14, 16: front psi S v | Y (stages 2, 3) or Q (stage 4)
+    return (STAGE == 11 || STAGE == 16) ? 4 : 6;
   }
   return STAGE == 5 ? 3 : ((STAGE <= 1 || STAGE == 6) ? 4 : (STAGE == 4 ? 6 : 8));
 }
@@ -356,10 +354,11 @@ __global__ void __launch_bounds__((TW / VX) * BY,
   constexpr int NGA = G::NGA, SWA = G::SWA;
   constexpr int NGV = (NG + VX - 1) / VX * VX;  // halo rounded to whole vectors
   constexpr int NS = march_nstreams<STAGE>();
-  // STAGE >= 10: the ACC-free ("lean") arrangement of the same RK4 (variant 3): stage buffers hold
-  // Y1 = Y + dt/2 k1, Y2 = Y + dt/2 k2, Y3 = Y + dt k3 and stage 4 forms
-  // Y_new = (1/3)(-Y + Y1 + 2 Y2 + Y3) + dt/6 k4 -- 6w, 8w, 8w, 12w bytes per point instead of
-  // 8w, 12w, 12w, 8w, and no running sum in the DRAM-bound stages 2 and 3.
+  // STAGE >= 10: the ACC-free ("lean") arrangement of the same RK4 (the default): stage 1 writes
+  // Y1 = Y + dt/2 k1 (buffer A); stage 2 writes Y2 = Y + dt/2 k2 (B) and Q = (Y1 - Y) + 2 Y2 (the
+  // ACC buffer); stage 3 writes Y3 = Y + dt k3 (A again, Y1 is no longer needed); stage 4 forms
+  // Y_new = (1/3)(Q + Y3) + dt/6 k4 = Y + dt/6 (k1 + 2 k2 + 2 k3 + k4).  Bytes per point:
+  // 6w, 10w, 8w, 8w = 32w per step instead of 8w, 12w, 12w, 8w = 40w.
   constexpr bool LEAN = STAGE >= 10;
   constexpr int ST = STAGE % 10;
   constexpr int RK = ST == 6 ? 1 : ST;                  // which RK combine (0 = store k)
@@ -368,11 +367,9 @@ __global__ void __launch_bounds__((TW / VX) * BY,
   // slots of the pointwise boxes (lean: Y right after v, then Y1, then Y2)
   constexpr int S_YU = LEAN ? 4 : ST_YU, S_YV = LEAN ? 5 : ST_YV;
   constexpr int S_AU = LEAN ? 6 : ST_AU, S_AV = LEAN ? 7 : ST_AV;
-  constexpr int S_BU = 8, S_BV = 9;
-  constexpr bool NEED_Y = (RK == 2 || RK == 3) || (LEAN && RK == 4);
-  constexpr bool NEED_A = LEAN ? RK == 4 : (RK >= 2 && RK <= 4);
-  constexpr bool NEED_B = LEAN && RK == 4;
-  constexpr bool WRITE_ACC = !LEAN && RK >= 1 && RK <= 3;
+  constexpr bool NEED_Y = (RK == 2 || RK == 3) || (LEAN && RK == 4);  // lean stage 4: the Y slot is Q
+  constexpr bool NEED_A = !LEAN && RK >= 2 && RK <= 4;
+  constexpr bool WRITE_ACC = LEAN ? RK == 2 : (RK >= 1 && RK <= 3);   // lean stage 2: ACC <- Q
   constexpr bool PACKED = HR_MARCH_F32X2 && sizeof(T) == 4 && VX == 2;  // FFMA2 / FADD2 path
   constexpr int RING = D + 1;
   constexpr int SLOT_BYTES = G::TILE_BYTES + NS * G::BOX_BYTES;
@@ -651,7 +648,7 @@ __global__ void __launch_bounds__((TW / VX) * BY,
           }
           if constexpr (ADVANCE) {
             const V vin = *reinterpret_cast<const V*>(sb + ST_V * (TW * BY) + so);
-            [[maybe_unused]] V yu{}, yv{}, au{}, av{}, bu{}, bv{};
+            [[maybe_unused]] V yu{}, yv{}, au{}, av{};
             if constexpr (NEED_A && !PACKED) {
               au = *reinterpret_cast<const V*>(sb + S_AU * (TW * BY) + so);
               av = *reinterpret_cast<const V*>(sb + S_AV * (TW * BY) + so);
@@ -660,10 +657,7 @@ __global__ void __launch_bounds__((TW / VX) * BY,
               yu = *reinterpret_cast<const V*>(sb + S_YU * (TW * BY) + so);
               yv = *reinterpret_cast<const V*>(sb + S_YV * (TW * BY) + so);
             }
-            if constexpr (NEED_B && !PACKED) {
-              bu = *reinterpret_cast<const V*>(sb + S_BU * (TW * BY) + so);
-              bv = *reinterpret_cast<const V*>(sb + S_BV * (TW * BY) + so);
-            }
+
             V wu, wv, nu, nv;  // stage output and the new running sum
             if constexpr (PACKED) {
               auto L2 = [](const T* q) { return F2{*reinterpret_cast<const unsigned long long*>(q)}; };
@@ -678,7 +672,7 @@ __global__ void __launch_bounds__((TW / VX) * BY,
               const F2 vin2 = L2(sb + ST_V * (TW * BY) + so);
               const F2 ku = f2_fma(f2_bc(-(float)a.eta), uc2, vin2);
               const F2 kv = f2_mul(c2p, H2);
-              F2 yu2{}, yv2{}, au2{}, av2{}, bu2{}, bv2{};
+              F2 yu2{}, yv2{}, au2{}, av2{};
               if constexpr (NEED_A) {
                 au2 = L2(sb + S_AU * (TW * BY) + so);
                 av2 = L2(sb + S_AV * (TW * BY) + so);
@@ -687,14 +681,14 @@ __global__ void __launch_bounds__((TW / VX) * BY,
                 yu2 = L2(sb + S_YU * (TW * BY) + so);
                 yv2 = L2(sb + S_YV * (TW * BY) + so);
               }
-              if constexpr (NEED_B) {
-                bu2 = L2(sb + S_BU * (TW * BY) + so);
-                bv2 = L2(sb + S_BV * (TW * BY) + so);
-              }
               F2 wu2, wv2, nu2{}, nv2{};
               if constexpr (LEAN) {
-                wu2 = rk_lean_f2<RK>((float)a.dt, ku, uc2, yu2, au2, bu2);
-                wv2 = rk_lean_f2<RK>((float)a.dt, kv, vin2, yv2, av2, bv2);
+                wu2 = rk_lean_f2<RK>((float)a.dt, ku, uc2, yu2);
+                wv2 = rk_lean_f2<RK>((float)a.dt, kv, vin2, yv2);
+                if constexpr (RK == 2) {  // Q = (Y1 - Y) + 2 Y2
+                  nu2 = f2_add(f2_sub(uc2, yu2), f2_add(wu2, wu2));
+                  nv2 = f2_add(f2_sub(vin2, yv2), f2_add(wv2, wv2));
+                }
               } else {
                 rk_values_f2<RK>((float)a.dt, ku, kv, uc2, vin2, yu2, yv2, au2, av2, wu2, wv2, nu2, nv2);
               }
@@ -709,8 +703,12 @@ __global__ void __launch_bounds__((TW / VX) * BY,
                 const T ku = vin.v[j] - a.eta * uc;
                 const T kv = c2[j] * H[j];
                 if constexpr (LEAN) {
-                  wu.v[j] = rk_lean<T, RK>(a.dt, ku, uc, yu.v[j], au.v[j], bu.v[j]);
-                  wv.v[j] = rk_lean<T, RK>(a.dt, kv, vin.v[j], yv.v[j], av.v[j], bv.v[j]);
+                  wu.v[j] = rk_lean<T, RK>(a.dt, ku, uc, yu.v[j]);
+                  wv.v[j] = rk_lean<T, RK>(a.dt, kv, vin.v[j], yv.v[j]);
+                  if constexpr (RK == 2) {  // Q = (Y1 - Y) + 2 Y2
+                    nu.v[j] = (uc - yu.v[j]) + (wu.v[j] + wu.v[j]);
+                    nv.v[j] = (vin.v[j] - yv.v[j]) + (wv.v[j] + wv.v[j]);
+                  }
                 } else {
                   rk_values<T, RK>(a.dt, ku, kv, uc, vin.v[j], yu.v[j], yv.v[j], au.v[j], av.v[j],
                                    wu.v[j], wv.v[j], nu.v[j], nv.v[j]);
@@ -860,14 +858,16 @@ __global__ void __launch_bounds__((TW / VX) * BY,
       const T kv = radiation_k(a.in_v, c, g.P0, r0, r1, ri);
       T wu, wv;
       if constexpr (LEAN) {
-        T yu = T(0), yv = T(0), au = T(0), av = T(0), bu = T(0), bv = T(0);
-        if constexpr (NEED_Y) { yu = a.y_u[c]; yv = a.y_v[c]; }
-        if constexpr (NEED_A) { au = a.acc_u[c]; av = a.acc_v[c]; }  // lean stage 4: Y1 (buffer A)
-        if constexpr (NEED_B) { bu = a.b_u[c]; bv = a.b_v[c]; }      // lean stage 4: Y2 (buffer B)
-        wu = rk_lean<T, RK>(a.dt, ku, uc, yu, au, bu);
-        wv = rk_lean<T, RK>(a.dt, kv, vc, yv, av, bv);
+        T yu = T(0), yv = T(0);
+        if constexpr (NEED_Y) { yu = a.y_u[c]; yv = a.y_v[c]; }  // lean stage 4: y_u / y_v point at Q
+        wu = rk_lean<T, RK>(a.dt, ku, uc, yu);
+        wv = rk_lean<T, RK>(a.dt, kv, vc, yv);
         a.out_u[c] = wu;
         a.out_v[c] = wv;
+        if constexpr (RK == 2) {
+          a.acc_u[c] = (uc - yu) + (wu + wu);
+          a.acc_v[c] = (vc - yv) + (wv + wv);
+        }
       } else {
         rk_combine<T, RK>(a, c, ku, kv, uc, vc, wu, wv);
       }
