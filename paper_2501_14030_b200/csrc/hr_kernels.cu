@@ -637,6 +637,9 @@ static void choose_chunks(MarchPlan& m, int n2, int ng, int slots, bool f64) {
     zc = std::atoi(zc_env);
   } else {
     const long long ntiles = (long long)m.ntx * m.nty;
+    // fp64 with plenty of items (>= 4 rounds): 12 planes amortise the window priming better
+    // (config 3: +1.5 %, 512x256x256: +3 %; on 128^3 8 planes stay ahead)
+    if (f64 && ntiles * ((n2 + 11) / 12) >= 4LL * slots) zc = 12;
     while (zc > 2 && ntiles * ((n2 + zc - 1) / zc) < slots) --zc;
   }
   if (zc > n2) zc = n2;
