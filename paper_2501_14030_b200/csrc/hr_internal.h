@@ -113,7 +113,7 @@ struct HrArrays {
 #define HR_MARCH_D_F64 2
 #endif
 #ifndef HR_MARCH_D_EXTRA_LIGHT
-#define HR_MARCH_D_EXTRA_LIGHT 1
+#define HR_MARCH_D_EXTRA_LIGHT 0
 #endif
 #ifndef HR_MARCH_D_F32
 #define HR_MARCH_D_F32 2

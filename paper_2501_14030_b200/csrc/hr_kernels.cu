@@ -578,9 +578,10 @@ struct MarchCfg<float> {
   static constexpr int TW = HR_TW_F32, BY = HR_BY_F32, VX = HR_VX_F32, D = HR_MARCH_D_F32;
 };
 
-// Planes of look-ahead: the DRAM-bound stages 2 and 3 (12 w bytes per point) do best with D; in
-// fp64 the lighter kernels (8 w and the residual) gain 1-3 % from one plane more, in fp32 they
-// do not (measured on config 3).
+// Planes of look-ahead.  D = 2 everywhere by default (D = 1: -7 %).  HR_MARCH_D_EXTRA_LIGHT adds
+// planes for the fp64 kernels other than the heaviest: with the running-sum arrangement
+// (variant 3) one more plane gained 1-3 % on the 8 w kernels; with the default arrangement, whose
+// kernels are all bound by the plane loop, it costs 1 % (shared memory -> occupancy), so it is 0.
 template <typename T, int STAGE>
 constexpr int march_depth() {
   // (the heavy kernels: stages 2, 3 of the running-sum form, 12 w; stage 2 = code 12 of the
