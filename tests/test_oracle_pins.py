@@ -1,4 +1,4 @@
-"""Pins P1-P12 (SURVEY.md Sec. 8c / DESIGN.md): the CPU oracle checked against what the paper and
+"""Pins P1-P14 (SURVEY.md Sec. 8c / DESIGN.md): the CPU oracle checked against what the paper and
 the mathematics fix -- closed forms, invariants, textbook identities, brute force -- never
 against itself.  CPU only (`-m "not gpu"`).
 """
@@ -596,3 +596,102 @@ def test_invalid_parameters_are_rejected():
         p.update(bad)
         with pytest.raises(ValueError):
             O.Oracle(p)
+
+
+# ------------------------------------------------------------------------------------------
+# P13  the grid-centre offset `origin` (C6): every other pin runs with origin = 0
+# ------------------------------------------------------------------------------------------
+def test_p13_origin_offset_enters_the_sources_with_the_right_sign_and_axis():
+    """psi_BL and S on a grid whose centre is NOT the Cartesian origin equal the closed forms at
+    (coordinate map + origin): a sign slip (map - origin) or an axis slip fails, because the three
+    components of origin differ and the punctures sit off every axis."""
+    ckw = dict(coord="SinhSymTP", amp=8.0, sinhw=0.8, bscale=2.0)
+    origin = (0.3, -0.2, -3.0)
+    P, S, pos, m = np.array([0.05, -0.02, 0.11]), np.array([0.1, 0.05, -0.2]), np.array([0.4, 0.7, -1.1]), 0.6
+    p = small(ckw, (12, 10, 8), 4, punctures=[[m, *pos, *P, *S]], origin=origin)
+    o = O.Oracle(p)
+    psi, Ssrc = o.source()
+    x0, x1, x2 = o.coords()
+    # Cartesian position written out here (not through grid_cart / the oracle's map): C4 + C6
+    A = p["amp"] * np.sinh(x0 / p["sinhw"]) / np.sinh(1 / p["sinhw"])
+    X = A[None, None, :] * np.sin(x1)[None, :, None] * np.cos(x2)[:, None, None] + origin[0]
+    Y = A[None, None, :] * np.sin(x1)[None, :, None] * np.sin(x2)[:, None, None] + origin[1]
+    Z = np.sqrt(A**2 + p["bscale"] ** 2)[None, None, :] * np.cos(x1)[None, :, None] * np.ones_like(x2)[:, None, None] + origin[2]
+    d = np.stack([X - pos[0], Y - pos[1], Z - pos[2]], axis=-1).reshape(-1, 3)
+    r = np.linalg.norm(d, axis=1)
+    n = d / r[:, None]
+    assert np.allclose(psi, 1 + m / (2 * r), rtol=1e-13)
+    closed = (9 / (2 * r**4) * (P @ P + 2 * (n @ P) ** 2) + 18 / r**6 * (S @ S - (n @ S) ** 2)
+              + 18 / r**5 * (np.cross(S, n) @ P))
+    assert np.allclose(Ssrc, closed / 8, rtol=1e-10)
+    # and the wrong readings are far outside that tolerance (the test can tell them apart)
+    for wrong in ((-0.3, 0.2, 3.0), (-3.0, -0.2, 0.3), (0.0, 0.0, 0.0)):
+        dw = d - np.asarray(origin) + np.asarray(wrong)
+        assert not np.allclose(psi, 1 + m / (2 * np.linalg.norm(dw, axis=1)), rtol=1e-3)
+
+
+def test_p13_config3_foci_sit_on_the_punctures():
+    """C6 for configs[3]: origin = (0,0,-3), b = 5 puts the SymTP foci (grid z = +-b) on the
+    punctures at z = +2 and z = -8, so psi_BL peaks at the grid points next to each focus:
+    smallest rho, theta next to 0 (upper focus) or pi (lower focus).  With the sign of origin
+    flipped the foci would sit at z = +8 and -2 and the maxima would move."""
+    p = W.config(3, scale=0.0625)
+    o = O.Oracle(p)
+    psi, _ = o.source()
+    ng = o.ng
+    P3 = psi.reshape(o.T[2], o.T[1], o.T[0])[ng:-ng, ng:-ng, ng:-ng]
+    n2, n1, n0 = P3.shape
+    upper, lower = P3[:, : n1 // 2, :], P3[:, n1 // 2:, :]
+    ku = np.unravel_index(np.argmax(upper), upper.shape)
+    kl = np.unravel_index(np.argmax(lower), lower.shape)
+    assert ku[1:] == (0, 0) and kl[1:] == (n1 - n1 // 2 - 1, 0), (ku, kl)
+    # the heavier puncture (m = 0.8) is the upper one, and both peaks dwarf the far field
+    assert upper.max() - 1 > lower.max() - 1 > 100 * (np.median(P3) - 1)
+
+
+# ------------------------------------------------------------------------------------------
+# P14  the d_theta part of d_r in SinhSymTP (rad1 of C13) where it matters
+# ------------------------------------------------------------------------------------------
+def test_p14_symtp_radial_derivative_theta_term_at_order_one():
+    """P9 again on a SymTP grid whose outer boundary lies at A ~ b, where
+    d_r f = rad0 d_0 f + rad1 d_1 f has a theta part of order one (in P9 it is < 1 %).  The
+    outgoing wave G(r - t)/r is still annihilated at second order, and the converged error is a
+    small fraction of the theta term itself -- so dropping rad1 (error = the term) or flipping
+    its sign (error = twice the term) cannot pass."""
+    ckw = dict(coord="SinhSymTP", amp=3.0, sinhw=0.9, bscale=3.0)
+    r0, sig = 3.4, 1.6
+
+    def G(r):
+        return np.exp(-((r - r0) / sig) ** 2)
+
+    def dG(r):
+        return -2 * (r - r0) / sig**2 * G(r)
+
+    errs, theta_share = [], []
+    for n in ((24, 16, 8), (48, 32, 8), (96, 64, 8)):
+        p = small(ckw, n, 4)
+        o = O.Oracle(p)
+        xyz = grid_cart(o, p)
+        r = np.linalg.norm(xyz, axis=1)
+        f = G(r) / r
+        ku, _ = o.rhs(f, f, part="outer")
+        _, _, outer = o.bc_lists()
+        c = np.broadcast_to(o.planes()["c"][None], (o.T[2], o.T[1], o.T[0])).reshape(-1)
+        exact = -c * dG(r) / r
+        scale = np.max(np.abs(exact[outer]))
+        errs.append(np.max(np.abs(ku[outer] - exact[outer])) / scale)
+        # analytic size of the theta term: c * rad1 * d_theta f, with r^2 = A^2 + b^2 cos^2(theta)
+        # => d_theta r = -b^2 sin cos / r and rad1 = -b^2 sin cos / (r Sigma) (C13)
+        x0, x1, _ = o.coords()
+        A = p["amp"] * np.sinh(x0 / p["sinhw"]) / np.sinh(1 / p["sinhw"])
+        b2 = p["bscale"] ** 2
+        st, ct = np.sin(x1)[:, None], np.cos(x1)[:, None]
+        rr = np.sqrt(A[None, :] ** 2 + b2 * ct**2)
+        Sig = A[None, :] ** 2 + b2 * st**2
+        dfdr = dG(rr) / rr - G(rr) / rr**2
+        term = (-b2 * st * ct / (rr * Sig)) * dfdr * (-b2 * st * ct / rr)   # rad1 * d_theta f
+        term = np.broadcast_to((o.planes()["c"] * term)[None], (o.T[2], o.T[1], o.T[0])).reshape(-1)
+        theta_share.append(np.max(np.abs(term[outer])) / scale)
+    assert theta_share[-1] > 0.05, theta_share            # the term is not negligible here
+    assert errs[1] < errs[0] / 3.0 and errs[2] < errs[1] / 3.0, errs   # second order
+    assert errs[2] < 0.2 * theta_share[2], (errs, theta_share)         # far below the term itself
