@@ -103,6 +103,12 @@ struct HrArrays {
 #define HR_MARCH_F32X2 1
 #endif
 
+// 1: fp32 takes the increment-preserving ACC-free RK4 (stage codes 22 / 24: one rounding of the size of Y
+// per step, stage 4 reads Y as well: 34w instead of 32w bytes per point and step); 0: the plain form.
+#ifndef HR_F32_PRECISE_RK
+#define HR_F32_PRECISE_RK 1
+#endif
+
 // Copies of the plane-loop body per window shift (HR_MARCH_ROTATE = 0).
 #ifndef HR_MARCH_UNROLL
 #define HR_MARCH_UNROLL 2

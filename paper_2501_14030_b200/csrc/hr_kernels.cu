@@ -456,13 +456,15 @@ StepArgs<T> make_args(const hr_solver* s, int stage, void* ku, void* kv) {
     case 16:  // lean: Y -> Y1 (A)
       r.in_u = P(a.Y[0]); r.in_v = P(a.Y[1]); r.out_u = P(a.A[0]); r.out_v = P(a.A[1]);
       break;
-    case 12:  // lean: Y1 (A) -> Y2 (B)
+    case 12:
+    case 22:  // lean: Y1 (A) -> Y2 (B)
       r.in_u = P(a.A[0]); r.in_v = P(a.A[1]); r.out_u = P(a.B[0]); r.out_v = P(a.B[1]);
       break;
     case 13:  // lean: Y2 (B) -> Y3 (A again: Y1 is no longer needed)
       r.in_u = P(a.B[0]); r.in_v = P(a.B[1]); r.out_u = P(a.A[0]); r.out_v = P(a.A[1]);
       break;
-    case 14:  // lean: Y3 (A) -> Y, reading Q (the ACC buffer)
+    case 14:
+    case 24:  // lean: Y3 (A) -> Y, reading Q (the ACC buffer); 24 also reads Y
       r.in_u = P(a.A[0]); r.in_v = P(a.A[1]); r.out_u = P(a.Y[0]); r.out_v = P(a.Y[1]);
       break;
     default:  // 5, residual: the stencil source is the state
@@ -471,7 +473,7 @@ StepArgs<T> make_args(const hr_solver* s, int stage, void* ku, void* kv) {
   }
   r.y_u = P(a.Y[0]); r.y_v = P(a.Y[1]);
   r.acc_u = P(a.ACC[0]); r.acc_v = P(a.ACC[1]);
-  if (stage == 14) {  // Q rides in the Y slots
+  if (stage == 14) {  // Q rides in the Y slots (stage 24 keeps Y there and reads Qd from the ACC slots)
     r.y_u = P(a.ACC[0]); r.y_v = P(a.ACC[1]);
   }
   r.psi = P(a.psi); r.S = P(a.S);
@@ -590,6 +592,14 @@ constexpr int march_depth() {
          ((STAGE == 2 || STAGE == 3 || STAGE == 12 || sizeof(T) != 8) ? 0 : HR_MARCH_D_EXTRA_LIGHT);
 }
 
+// Stage codes of the default arrangement's stages 2 and 4 per dtype: fp32 takes the increment-preserving
+// forms 22 / 24 (hr_march.cuh: rk_prec_q, rk_prec_4), fp64 the plain ACC-free forms 12 / 14.
+template <typename T>
+struct LeanCode {
+  static constexpr bool PREC = sizeof(T) == 4 && HR_F32_PRECISE_RK;
+  static constexpr int S2 = PREC ? 22 : 12, S4 = PREC ? 24 : 14;
+};
+
 #define HR_MARCH_KERNEL(T, NG, STAGE) \
   k_march<T, NG, STAGE, MarchCfg<T>::TW, MarchCfg<T>::BY, MarchCfg<T>::VX, march_depth<T, STAGE>()>
 #define HR_MARCH_SMEM(T, NG, STAGE) \
@@ -696,9 +706,9 @@ cudaError_t prepare_march(hr_solver* s) {
   if ((e = prepare_march_stage<T, NG, 6>(s, &s->march_grid[6])) != cudaSuccess) return e;
   if (s->p.variant == 0) {  // the ACC-free arrangement's kernels, grid sizes indexed by stage % 10
     if ((e = prepare_march_stage<T, NG, 11>(s, &s->march_grid_lean[1])) != cudaSuccess) return e;
-    if ((e = prepare_march_stage<T, NG, 12>(s, &s->march_grid_lean[2])) != cudaSuccess) return e;
+    if ((e = prepare_march_stage<T, NG, LeanCode<T>::S2>(s, &s->march_grid_lean[2])) != cudaSuccess) return e;
     if ((e = prepare_march_stage<T, NG, 13>(s, &s->march_grid_lean[3])) != cudaSuccess) return e;
-    if ((e = prepare_march_stage<T, NG, 14>(s, &s->march_grid_lean[4])) != cudaSuccess) return e;
+    if ((e = prepare_march_stage<T, NG, LeanCode<T>::S4>(s, &s->march_grid_lean[4])) != cudaSuccess) return e;
     if ((e = prepare_march_stage<T, NG, 16>(s, &s->march_grid_lean[6])) != cudaSuccess) return e;
   }
   // one chunking for all stages, balanced for the RK stage kernels (stages 2, 3 dominate)
@@ -727,9 +737,10 @@ cudaError_t prepare_march_ng(hr_solver* s) {
 // Tensor maps of one stage: stencil source = Y (stages 0, 1, residual), A (2, 4), B (3).
 MarchMaps make_maps(const hr_solver* s, int stage) {
   MarchMaps m;
-  if (stage >= 10) {  // lean: front psi S v | Y (stages 2, 3) or Q = ACC (stage 4); sources Y, A, B, A
-    const int in = (stage == 12 || stage == 14) ? 1 : (stage == 13 ? 2 : 0);
-    const int ys = stage == 14 ? 6 : 0;
+  if (stage >= 10) {  // lean: front psi S v | Y (stages 2, 3) or Q = ACC (stage 4) | Y; sources Y, A, B, A
+    const int st = stage % 10;
+    const int in = (st == 2 || st == 4) ? 1 : (st == 3 ? 2 : 0);
+    const int ys = st == 4 ? 6 : 0;
     m.tile = s->tm_tile[in];
     m.st[0] = s->tm_box[2 * in];
     m.st[1] = s->tm_box[8];
@@ -738,7 +749,7 @@ MarchMaps make_maps(const hr_solver* s, int stage) {
     m.st[4] = s->tm_box[ys];
     m.st[5] = s->tm_box[ys + 1];
     m.st[6] = s->tm_box[0];
-    m.st[7] = s->tm_box[0];
+    m.st[7] = s->tm_box[1];
     return m;
   }
   const int in = (stage == 2 || stage == 4) ? 1 : (stage == 3 ? 2 : 0);  // 0, 1, 5, 6: Y
@@ -768,6 +779,8 @@ cudaError_t launch_march_stage(const hr_solver* s, const StepArgs<T>& a, const R
 template <typename T, int NG>
 cudaError_t launch_march(const hr_solver* s, int stage, void* ku, void* kv, int mode,
                          double* partials, double* out2 = nullptr) {
+  if (stage == 12) stage = LeanCode<T>::S2;
+  if (stage == 14) stage = LeanCode<T>::S4;
   const StepArgs<T> a = make_args<T>(s, stage, ku, kv);
   const ResidArgs ra{s->a.Wvol, partials, mode, out2};
   switch (stage) {
@@ -778,9 +791,11 @@ cudaError_t launch_march(const hr_solver* s, int stage, void* ku, void* kv, int 
     case 4: return launch_march_stage<T, NG, 4>(s, a, ra);
     case 6: return launch_march_stage<T, NG, 6>(s, a, ra);
     case 11: return launch_march_stage<T, NG, 11>(s, a, ra);
-    case 12: return launch_march_stage<T, NG, 12>(s, a, ra);
+    case 12:
+    case 22: return launch_march_stage<T, NG, LeanCode<T>::S2>(s, a, ra);
     case 13: return launch_march_stage<T, NG, 13>(s, a, ra);
-    case 14: return launch_march_stage<T, NG, 14>(s, a, ra);
+    case 14:
+    case 24: return launch_march_stage<T, NG, LeanCode<T>::S4>(s, a, ra);
     case 16: return launch_march_stage<T, NG, 16>(s, a, ra);
     default: return launch_march_stage<T, NG, 5>(s, a, ra);
   }

@@ -124,6 +124,29 @@ __device__ __forceinline__ F2 rk_lean_f2(float dt, F2 k, F2 in, F2 y) {
   return f2_fma(f2_bc(dt / 6.f), k, f2_mul(f2_bc(1.f / 3.f), f2_add(y, in)));
 }
 
+// The increment-preserving form of the same arrangement (STAGE >= 20; the fp32 default): stage 2 keeps
+// Qd = (Y1 - Y) + dt k2 -- an increment, so its rounding error is relative to dt k, not to Y -- and
+// stage 4 adds increments to Y:  Y_new = Y + [ (1/3)(Qd + (Y3 - Y)) + dt/6 k4 ].  One rounding at the
+// size of Y per step, like the textbook k-sum form, at the price of reading Y in stage 4 (10w instead
+// of 8w in that stage).  In the plain ACC-free form the roundings of Q = (Y1 - Y) + 2 Y2, of Q + Y3
+// and of the product by 1/3 are each of the size of ulp(Y): twice the per-step noise in the state,
+// which the residual amplifies by 1/ds^2 (fp32: visible against the 1e-4 bar of reading C21).
+template <typename T>
+__device__ __forceinline__ T rk_prec_q(T dt, T k, T in, T y) {
+  return (in - y) + dt * k;
+}
+template <typename T>
+__device__ __forceinline__ T rk_prec_4(T dt, T k, T in, T q, T y) {
+  return y + ((T(1) / T(3)) * (q + (in - y)) + dt / T(6) * k);
+}
+__device__ __forceinline__ F2 rk_prec_q_f2(float dt, F2 k, F2 in, F2 y) {
+  return f2_fma(f2_bc(dt), k, f2_sub(in, y));
+}
+__device__ __forceinline__ F2 rk_prec_4_f2(float dt, F2 k, F2 in, F2 q, F2 y) {
+  const F2 t = f2_mul(f2_bc(1.f / 3.f), f2_add(q, f2_sub(in, y)));
+  return f2_add(y, f2_fma(f2_bc(dt / 6.f), k, t));
+}
+
 // Tensor maps of one launch: the halo-tile box of the stage's u and the TW x BY box of every
 // pointwise input, indexed by ST_*.
 struct alignas(64) MarchMaps {
@@ -311,7 +334,8 @@ enum { ST_FRONT = 0, ST_PSI = 1, ST_S = 2, ST_V = 3, ST_AU = 4, ST_AV = 5, ST_YU
 template <int STAGE>
 __host__ __device__ constexpr int march_nstreams() {
   if (STAGE >= 10) {  // ACC-free stages 11..14, 16: front psi S v | Y (stages 2, 3) or Q (stage 4)
-    return (STAGE == 11 || STAGE == 16) ? 4 : 6;
+    if (STAGE == 24) return 8;  // increment-preserving stage 4: ... | Qd | Y
+    return (STAGE % 10 == 1 || STAGE % 10 == 6) ? 4 : 6;
   }
   return STAGE == 5 ? 3 : ((STAGE <= 1 || STAGE == 6) ? 4 : (STAGE == 4 ? 6 : 8));
 }
@@ -360,6 +384,7 @@ __global__ void __launch_bounds__((TW / VX) * BY,
   // Y_new = (1/3)(Q + Y3) + dt/6 k4 = Y + dt/6 (k1 + 2 k2 + 2 k3 + k4).  Bytes per point:
   // 6w, 10w, 8w, 8w = 32w per step instead of 8w, 12w, 12w, 8w = 40w.
   constexpr bool LEAN = STAGE >= 10;
+  constexpr bool PREC = STAGE >= 20;  // increment-preserving stages 22 and 24 (rk_prec_q, rk_prec_4)
   constexpr int ST = STAGE % 10;
   constexpr int RK = ST == 6 ? 1 : ST;                  // which RK combine (0 = store k)
   constexpr bool RESID = ST == 5 || ST == 6;            // accumulate sum w H^2, sum w
@@ -368,7 +393,7 @@ __global__ void __launch_bounds__((TW / VX) * BY,
   constexpr int S_YU = LEAN ? 4 : ST_YU, S_YV = LEAN ? 5 : ST_YV;
   constexpr int S_AU = LEAN ? 6 : ST_AU, S_AV = LEAN ? 7 : ST_AV;
   constexpr bool NEED_Y = (RK == 2 || RK == 3) || (LEAN && RK == 4);  // lean stage 4: the Y slot is Q
-  constexpr bool NEED_A = !LEAN && RK >= 2 && RK <= 4;
+  constexpr bool NEED_A = (!LEAN && RK >= 2 && RK <= 4) || (PREC && RK == 4);  // PREC stage 4: the A slot is Y
   constexpr bool WRITE_ACC = LEAN ? RK == 2 : (RK >= 1 && RK <= 3);   // lean stage 2: ACC <- Q
   constexpr bool PACKED = HR_MARCH_F32X2 && sizeof(T) == 4 && VX == 2;  // FFMA2 / FADD2 path
   constexpr int RING = D + 1;
@@ -683,9 +708,17 @@ __global__ void __launch_bounds__((TW / VX) * BY,
               }
               F2 wu2, wv2, nu2{}, nv2{};
               if constexpr (LEAN) {
-                wu2 = rk_lean_f2<RK>((float)a.dt, ku, uc2, yu2);
-                wv2 = rk_lean_f2<RK>((float)a.dt, kv, vin2, yv2);
-                if constexpr (RK == 2) {  // Q = (Y1 - Y) + 2 Y2
+                if constexpr (PREC && RK == 4) {
+                  wu2 = rk_prec_4_f2((float)a.dt, ku, uc2, yu2, au2);
+                  wv2 = rk_prec_4_f2((float)a.dt, kv, vin2, yv2, av2);
+                } else {
+                  wu2 = rk_lean_f2<RK>((float)a.dt, ku, uc2, yu2);
+                  wv2 = rk_lean_f2<RK>((float)a.dt, kv, vin2, yv2);
+                }
+                if constexpr (RK == 2 && PREC) {  // Qd = (Y1 - Y) + dt k2
+                  nu2 = rk_prec_q_f2((float)a.dt, ku, uc2, yu2);
+                  nv2 = rk_prec_q_f2((float)a.dt, kv, vin2, yv2);
+                } else if constexpr (RK == 2) {  // Q = (Y1 - Y) + 2 Y2
                   nu2 = f2_add(f2_sub(uc2, yu2), f2_add(wu2, wu2));
                   nv2 = f2_add(f2_sub(vin2, yv2), f2_add(wv2, wv2));
                 }
@@ -703,9 +736,17 @@ __global__ void __launch_bounds__((TW / VX) * BY,
                 const T ku = vin.v[j] - a.eta * uc;
                 const T kv = c2[j] * H[j];
                 if constexpr (LEAN) {
-                  wu.v[j] = rk_lean<T, RK>(a.dt, ku, uc, yu.v[j]);
-                  wv.v[j] = rk_lean<T, RK>(a.dt, kv, vin.v[j], yv.v[j]);
-                  if constexpr (RK == 2) {  // Q = (Y1 - Y) + 2 Y2
+                  if constexpr (PREC && RK == 4) {
+                    wu.v[j] = rk_prec_4<T>(a.dt, ku, uc, yu.v[j], au.v[j]);
+                    wv.v[j] = rk_prec_4<T>(a.dt, kv, vin.v[j], yv.v[j], av.v[j]);
+                  } else {
+                    wu.v[j] = rk_lean<T, RK>(a.dt, ku, uc, yu.v[j]);
+                    wv.v[j] = rk_lean<T, RK>(a.dt, kv, vin.v[j], yv.v[j]);
+                  }
+                  if constexpr (RK == 2 && PREC) {  // Qd = (Y1 - Y) + dt k2
+                    nu.v[j] = rk_prec_q<T>(a.dt, ku, uc, yu.v[j]);
+                    nv.v[j] = rk_prec_q<T>(a.dt, kv, vin.v[j], yv.v[j]);
+                  } else if constexpr (RK == 2) {  // Q = (Y1 - Y) + 2 Y2
                     nu.v[j] = (uc - yu.v[j]) + (wu.v[j] + wu.v[j]);
                     nv.v[j] = (vin.v[j] - yv.v[j]) + (wv.v[j] + wv.v[j]);
                   }
@@ -860,11 +901,19 @@ __global__ void __launch_bounds__((TW / VX) * BY,
       if constexpr (LEAN) {
         T yu = T(0), yv = T(0);
         if constexpr (NEED_Y) { yu = a.y_u[c]; yv = a.y_v[c]; }  // lean stage 4: y_u / y_v point at Q
-        wu = rk_lean<T, RK>(a.dt, ku, uc, yu);
-        wv = rk_lean<T, RK>(a.dt, kv, vc, yv);
+        if constexpr (PREC && RK == 4) {  // Qd from the ACC buffer, Y through y_u / y_v
+          wu = rk_prec_4<T>(a.dt, ku, uc, a.acc_u[c], yu);
+          wv = rk_prec_4<T>(a.dt, kv, vc, a.acc_v[c], yv);
+        } else {
+          wu = rk_lean<T, RK>(a.dt, ku, uc, yu);
+          wv = rk_lean<T, RK>(a.dt, kv, vc, yv);
+        }
         a.out_u[c] = wu;
         a.out_v[c] = wv;
-        if constexpr (RK == 2) {
+        if constexpr (RK == 2 && PREC) {
+          a.acc_u[c] = rk_prec_q<T>(a.dt, ku, uc, yu);
+          a.acc_v[c] = rk_prec_q<T>(a.dt, kv, vc, yv);
+        } else if constexpr (RK == 2) {
           a.acc_u[c] = (uc - yu) + (wu + wu);
           a.acc_v[c] = (vc - yv) + (wv + wv);
         }
