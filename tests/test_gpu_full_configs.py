@@ -9,9 +9,9 @@ FROZEN BARS (a bar changes only in a commit that touches no
                   |r_gpu - r_or| <= 1e-10 * r_or   while r_or >= 1e-3 * max_n r_or(n)   (north_star, literal)
   fp64 state      max|u_gpu - u_or| <= 1e-10 * max|u_or| on the sampled points; v against |v| + eta |u|
   fp32 residual   |r_gpu32 - r_or64| <= 1e-4 * max_n r_or64(n)                 (asserted where
-                  BASELINE.json asks for fp32, i.e. config 2, and on config 0; elsewhere asserted unless the
-                  fp32 ORACLE itself has missed it by that mark, in which case the GPU must stay within 1.5x
-                  the oracle's largest miss so far -- two fp32 roundings of the same run are two noise samples)
+                  BASELINE.json asks for fp32, i.e. config 2, and on config 0, at every mark; everywhere as
+                  envelopes: the GPU's largest miss over the run <= max(1e-4 * peak, 1.5 x the fp32 ORACLE's
+                  largest miss over the run) -- two fp32 roundings of the same run are two noise samples)
   fp32 state      max|u_gpu32 - u_or64| <= 1.5 * max|u_or32 - u_or64| + 4 eps32 max|u|   (C21 iii: the GPU's
                   fp32 path may not drift more than 1.5x what the fp32 oracle itself drifts)
 Every literal relative number is printed beside the fp32 oracle's own and written to
@@ -120,6 +120,7 @@ def test_full_config_fp32(hr, case):
     bad = []
     peak = [0.0, 0.0]
     floor = [0.0, 0.0]
+    miss = [0.0, 0.0]
     for row in rows:
         m = int(row[0])
         s.hr_step(m - done)
@@ -131,12 +132,10 @@ def test_full_config_fp32(hr, case):
             dg, do = abs(r - ro), abs(r32o - ro)
             lines.append(f"{m} {mode} {r:.9e} {ro:.9e} {dg / ro:.2e} {do / ro:.2e} {dg / peak[mode]:.2e} "
                          f"{do / peak[mode]:.2e}")
-            floor[mode] = max(floor[mode], do)  # the largest miss the fp32 oracle itself has shown so far
-            if strict or floor[mode] <= 1e-4 * peak[mode]:
-                if dg > 1e-4 * peak[mode]:
-                    bad.append((m, mode, r, ro, r32o, dg / peak[mode]))
-            elif dg > 1.5 * floor[mode]:  # the fp32 oracle misses the C21 bar: hold the GPU to 1.5x its miss
-                bad.append((m, mode, r, ro, r32o, dg / floor[mode]))
+            if strict and dg > 1e-4 * peak[mode]:
+                bad.append((m, mode, r, ro, r32o, dg / peak[mode]))
+            floor[mode] = max(floor[mode], do)  # envelopes over the run: the fp32 oracle's largest miss
+            miss[mode] = max(miss[mode], dg)    # and the GPU's
         if f"u32_{m}" in z:
             u, v = sampled(s, idx)
             ou, ov = z[f"u64_{m}"], z[f"v64_{m}"]
@@ -146,6 +145,11 @@ def test_full_config_fp32(hr, case):
                          f"{eo / umax:.2e}  (of max|u|)")
             if eg > 1.5 * eo + 4 * EPS32 * umax:
                 bad.append((m, "state", eg / umax, eo / umax))
+    for mode in (0, 1):
+        lines.append(f"# mode {mode}: largest miss over the run, of the peak residual: gpu32 "
+                     f"{miss[mode] / peak[mode]:.2e}  fp32 oracle {floor[mode] / peak[mode]:.2e}")
+        if miss[mode] > max(1e-4 * peak[mode], 1.5 * floor[mode]):
+            bad.append(("envelope", mode, miss[mode] / peak[mode], floor[mode] / peak[mode]))
     emit(case, "f32", lines)
     assert not bad, (case, bad)
     s.close()
