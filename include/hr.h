@@ -217,6 +217,34 @@ HR_API hr_status hr_profile_step(hr_solver* s, int64_t n_steps, int32_t with_res
 /* Number of kernel launches one hr_step(1) enqueues (for bench.py's gpu_launches). */
 HR_API hr_status hr_launches_per_step(hr_solver* s, int32_t* n);
 
+/* Execution facts of a solver, for callers that report what they timed (bench.py) -- SURVEY.md section 5
+ * ("failure detection": the optional device flag) and VERDICT r1 item 10.  *value (host) receives:
+ *   HR_Q_STEP_GRAPH     1 if hr_step replays a captured CUDA graph of the RK4 step, 0 if the capture failed
+ *                       at hr_create and hr_step falls back to plain launches of the same kernels
+ *   HR_Q_RESID_GRAPH    the same for hr_step_residual_async (bit 0: mode 0, bit 1: mode 1; captured on first use)
+ *   HR_Q_PERSISTENT     1 if hr_step / hr_relax run the single-launch persistent step kernel (small grids)
+ *   HR_Q_NUMERIC_FLAG   non-zero once a kernel of this solver has met psi_BL + u <= 0 or a non-finite value
+ *                       at an interior point (reads the device flag: synchronises the stream)
+ *   HR_Q_PLAN_ZC, HR_Q_PLAN_ITEMS, HR_Q_PLAN_GRID   planes per work item, work items and persistent CTAs
+ *                       of the substep kernel                                                         */
+typedef enum {
+  HR_Q_STEP_GRAPH = 0, HR_Q_RESID_GRAPH = 1, HR_Q_PERSISTENT = 2, HR_Q_NUMERIC_FLAG = 3,
+  HR_Q_PLAN_ZC = 4, HR_Q_PLAN_ITEMS = 5, HR_Q_PLAN_GRID = 6
+} hr_query_what;
+HR_API hr_status hr_query(hr_solver* s, int32_t what, int64_t* value);
+
+/* Measurement hooks for the secondary roofs SURVEY.md section 8(d) asks for (no solver needed; device index and
+ * cudaStream_t as in hr_params).
+ * hr_measure_alu_peak: register-resident FMA chains (8 independent chains per thread, 1024 threads per CTA,
+ *   8 CTAs per SM-slot wave), dtype HR_F64 or HR_F32; packed != 0 uses fma.rn.f32x2 (HR_F32 only).
+ *   *tflops (host) = 2 * FMAs / best-of-3 CUDA-event time.
+ * hr_measure_launch_floor: a CUDA graph of `nodes` dependent launches of an empty kernel of `grid` CTAs x
+ *   `block` threads, replayed `reps` times; *us_per_graph (host) = mean microseconds per replay: the floor
+ *   under a step of `nodes` launches, whatever the kernels do.  Both synchronise the stream.              */
+HR_API hr_status hr_measure_alu_peak(int32_t device, void* stream, int32_t dtype, int32_t packed, double* tflops);
+HR_API hr_status hr_measure_launch_floor(int32_t device, void* stream, int32_t nodes, int32_t grid,
+                                         int32_t block, int32_t reps, double* us_per_graph);
+
 /* Thread-local, static storage; never NULL. */
 HR_API const char* hr_last_error(void);
 

@@ -5,6 +5,6 @@ Importing the package loads libhr_b200.so and raises if it has not been built --
 CPU fallback (the CPU oracle under oracle/ is test infrastructure and is never imported here).
 """
 from .binding import (HR_F32, HR_F64, HR_SINHSPHERICAL, HR_SINHSYMTP, HrError, Solver,  # noqa: F401
-                      hr_host_setup, hr_params, hr_puncture, hr_step_many, hr_version, hr_workspace_bytes,
+                      hr_host_setup, hr_measure_alu_peak, hr_measure_launch_floor, hr_params, hr_puncture, hr_step_many, hr_version, hr_workspace_bytes,
                       lib,
                       make_params)

@@ -81,6 +81,9 @@ _SIGS = {
                     C.POINTER(_i32), C.POINTER(_i64)],
     "hr_launches_per_step": [_vp, C.POINTER(_i32)],
     "hr_profile_step": [_vp, _i64, _i32, C.POINTER(C.c_double)],
+    "hr_query": [_vp, _i32, C.POINTER(_i64)],
+    "hr_measure_alu_peak": [_i32, _vp, _i32, _i32, C.POINTER(C.c_double)],
+    "hr_measure_launch_floor": [_i32, _vp, _i32, _i32, _i32, _i32, C.POINTER(C.c_double)],
     "hr_host_setup": [C.POINTER(hr_params), C.POINTER(C.c_double), C.POINTER(C.c_double),
                       C.POINTER(_i64), C.POINTER(_i64), _vp, _vp, _vp, _vp, _vp],
 }
@@ -100,6 +103,30 @@ def hr_step_many(solvers, n_steps: int):
     """n_steps RK4 steps of every Solver in `solvers`, interleaved, each on its own stream."""
     arr = (_vp * len(solvers))(*[s._h for s in solvers])
     _check(lib.hr_step_many(arr, _i32(len(solvers)), _i64(int(n_steps))))
+
+
+HR_Q = {"step_graph": 0, "resid_graph": 1, "persistent": 2, "numeric_flag": 3, "plan_zc": 4, "plan_items": 5,
+        "plan_grid": 6}
+
+
+def hr_measure_alu_peak(dtype="f64", packed=False, device=0) -> float:
+    """TFLOP/s of register-resident FMA chains (include/hr.h: hr_measure_alu_peak)."""
+    import torch
+    out = C.c_double()
+    st = torch.cuda.current_stream(device).cuda_stream
+    _check(lib.hr_measure_alu_peak(_i32(device), _vp(st), _i32(0 if dtype == "f64" else 1), _i32(int(packed)),
+                                   C.byref(out)))
+    return out.value
+
+
+def hr_measure_launch_floor(nodes=4, grid=1, block=32, reps=200, device=0) -> float:
+    """Microseconds per replay of a graph of `nodes` dependent empty launches (include/hr.h)."""
+    import torch
+    out = C.c_double()
+    stream = torch.cuda.Stream(device)
+    _check(lib.hr_measure_launch_floor(_i32(device), _vp(stream.cuda_stream), _i32(nodes), _i32(grid),
+                                       _i32(block), _i32(reps), C.byref(out)))
+    return out.value
 
 
 def hr_version() -> str:
@@ -308,6 +335,11 @@ class Solver:
                             _i32(int(mode)), C.byref(done), C.byref(res), _vp(hist.ctypes.data), _i64(cap),
                             C.byref(nh)))
         return int(done.value), float(res.value), hist[:min(cap, int(nh.value))].copy()
+
+    def hr_query(self, what: str) -> int:
+        out = _i64()
+        _check(lib.hr_query(self._h, _i32(HR_Q[what]), C.byref(out)))
+        return out.value
 
     def hr_profile_step(self, n_steps: int, with_residual=True):
         """Mean ms per RK4 step in {stage 1..4 fused kernel, inner fills, residual}."""

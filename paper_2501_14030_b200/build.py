@@ -7,7 +7,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libhr_b200.so")
-SOURCES = ["hr_api.cu", "hr_kernels.cu"]
+SOURCES = ["hr_api.cu", "hr_kernels.cu", "hr_measure.cu"]
 HEADERS = ["hr_internal.h", "fd_tables.cuh", "hr_march.cuh", os.path.join(ROOT, "include", "hr.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--fmad=true"]
@@ -32,16 +32,19 @@ def _stale() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not _stale():
         return LIB
-    objs = []
-    for src in SOURCES:
+    objs, procs = [], []
+    for src in SOURCES:  # the translation units compile side by side
         obj = os.path.join(CSRC, src.replace(".cu", ".o"))
         # HR_NVCC_DEFS="-DHR_MARCH_D_F64=3 ...": tuning overrides of the macros in hr_internal.h
         cmd = [_nvcc(), *NVCC_FLAGS, *os.environ.get("HR_NVCC_DEFS", "").split(), "-c",
                os.path.join(CSRC, src), "-o", obj]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
-        subprocess.run(cmd, check=True)
+        procs.append((cmd, subprocess.Popen(cmd)))
         objs.append(obj)
+    for cmd, pr in procs:
+        if pr.wait() != 0:
+            raise subprocess.CalledProcessError(pr.returncode, cmd)
     tmp = LIB + f".tmp{os.getpid()}"
     subprocess.run([_nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", *objs,
                     "-o", tmp], check=True)

@@ -60,9 +60,13 @@ hr_status validate(const hr_params* p) {
     if (p->n[a] < ng)
       return fail(HR_ERR_INVALID_ARG, "n[%d] = %d is smaller than NG = %d", a, p->n[a], ng);
   if (p->n[2] % 2) return fail(HR_ERR_INVALID_ARG, "n[2] = %d must be even (C14)", p->n[2]);
-  const double tot = double(p->n[0] + 2 * ng) * double(p->n[1] + 2 * ng) * double(p->n[2] + 2 * ng);
-  if (tot * 1.25 + 1e6 >= 2147483647.0)
-    return fail(HR_ERR_INVALID_ARG, "grid exceeds int32 index range");
+  {  // the kernels index the PADDED layout (row pitch P0) with int32: bound that, not N_tot
+    int P0 = 0, off0 = 0;
+    hrk_row_geometry(p->n[0] + 2 * ng, ng, p->dtype == HR_F64 ? 8 : 4, &P0, &off0);
+    const double npad = double(P0) * double(p->n[1] + 2 * ng) * double(p->n[2] + 2 * ng + 1);
+    if (npad + 1e6 >= 2147483647.0)
+      return fail(HR_ERR_INVALID_ARG, "grid exceeds the int32 index range of the stored layout");
+  }
   if (!(p->amp > 0) || !(p->sinhw > 0)) return fail(HR_ERR_INVALID_ARG, "amp, sinhw must be > 0");
   if (p->coord == HR_SINHSYMTP && !(p->bscale > 0))
     return fail(HR_ERR_INVALID_ARG, "bscale must be > 0 for SinhSymTP");
@@ -426,7 +430,10 @@ hr_status hr_create(const hr_params* p, void* workspace_dev, size_t workspace_by
   a.partials = reinterpret_cast<double*>(base + L.off_partials);
   a.result2 = reinterpret_cast<double*>(base + L.off_result);
   s->plan.counters = reinterpret_cast<int*>(base + L.off_counters);
+  s->plan.flag = s->plan.counters + 62;
   HR_CUDA(cudaMemsetAsync(s->plan.counters, 0, 256, s->stream));
+  HR_CUDA(cudaHostAlloc(reinterpret_cast<void**>(&s->pinned), 8 * sizeof(double), cudaHostAllocDefault));
+  for (auto& e : s->relax_ev) HR_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
   a.rho = reinterpret_cast<double*>(base + L.off_rho);
   a.rhoz = reinterpret_cast<double*>(base + L.off_rhoz);
   a.sinth = reinterpret_cast<double*>(base + L.off_sinth);
@@ -436,6 +443,9 @@ hr_status hr_create(const hr_params* p, void* workspace_dev, size_t workspace_by
   a.punct = reinterpret_cast<double*>(base + L.off_punct);
 
   HR_CUDA(hrk_prepare(s));  // tensor maps, shared-memory opt-in, persistent grid sizes
+  if ((int64_t)s->plan.ntx * s->plan.nty * s->plan.nzc > s->max_partials)
+    return fail(HR_ERR_WORKSPACE, "internal: %lld work items but room for %d residual partials",
+                (long long)s->plan.ntx * s->plan.nty * s->plan.nzc, s->max_partials);
 
   // ---- Alg. 1 l.2-4 on the host ----
   HostSetup H;
@@ -545,6 +555,9 @@ hr_status hr_destroy(hr_solver* s) {
   if (s->step_graph) cudaGraphExecDestroy(s->step_graph);
   for (cudaGraphExec_t g : s->step_resid_graph)
     if (g) cudaGraphExecDestroy(g);
+  if (s->pinned) cudaFreeHost(s->pinned);
+  for (cudaEvent_t e : s->relax_ev)
+    if (e) cudaEventDestroy(e);
   delete s;
   return HR_OK;
 }
@@ -610,9 +623,12 @@ hr_status hr_residual_ex(hr_solver* s, int32_t mode, double* out3) {
   if (!s || !out3) return fail(HR_ERR_INVALID_ARG, "NULL argument");
   hr_status st = hr_residual_async(s, mode, s->a.result2);
   if (st != HR_OK) return st;
-  double h[2];
-  HR_CUDA(cudaMemcpyAsync(h, s->a.result2, sizeof(h), cudaMemcpyDeviceToHost, s->stream));
+  double* h = s->pinned + 4;  // pinned: {num, den}, then the numeric flag
+  int* flag = reinterpret_cast<int*>(s->pinned + 6);
+  HR_CUDA(cudaMemcpyAsync(h, s->a.result2, 2 * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+  HR_CUDA(cudaMemcpyAsync(flag, s->plan.flag, sizeof(int), cudaMemcpyDeviceToHost, s->stream));
   HR_CUDA(cudaStreamSynchronize(s->stream));
+  if (*flag) return fail(HR_ERR_NUMERIC, "psi_BL + u <= 0 or a non-finite value at an interior point");
   out3[0] = std::sqrt(h[0] / h[1]);
   out3[1] = h[0];
   out3[2] = h[1];
@@ -626,23 +642,19 @@ hr_status hr_relax(hr_solver* s, int64_t max_steps, int64_t check_every, double 
   if (max_steps < 0 || check_every < 1 || !(tol >= 0) || (mode != 0 && mode != 1))
     return fail(HR_ERR_INVALID_ARG, "need max_steps >= 0, check_every >= 1, tol >= 0, mode 0 or 1");
   if (history && history_cap < 0) return fail(HR_ERR_INVALID_ARG, "history_cap < 0");
-  // two pinned slots and two events: the host tests block k-1 while block k runs
-  struct Pinned {
-    double* h = nullptr;
-    cudaEvent_t ev[2] = {nullptr, nullptr};
-    ~Pinned() {
-      if (h) cudaFreeHost(h);
-      for (cudaEvent_t e : ev) if (e) cudaEventDestroy(e);
-    }
-  } pin;
-  HR_CUDA(cudaHostAlloc(reinterpret_cast<void**>(&pin.h), 4 * sizeof(double), cudaHostAllocDefault));
-  for (auto& e : pin.ev) HR_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+  // two pinned slots and two events (owned by the solver): the host tests block k-1 while block k runs
+  struct {
+    double* h;
+    cudaEvent_t* ev;
+  } pin{s->pinned, s->relax_ev};
   double* dev = s->a.result2 + 2;  // device slots {num, den} x 2 behind hr_residual's own pair
   int64_t done = 0, nh = 0, k = 0;
+  double last_r = 0.0;
   bool met = false;
   auto test_block = [&](int64_t kk) -> hr_status {
     HR_CUDA(cudaEventSynchronize(pin.ev[kk & 1]));
     const double r = std::sqrt(pin.h[2 * (kk & 1)] / pin.h[2 * (kk & 1) + 1]);
+    last_r = r;
     if (history && nh < history_cap) history[nh] = r;
     ++nh;
     if (tol > 0 && r <= tol) met = true;
@@ -670,15 +682,14 @@ hr_status hr_relax(hr_solver* s, int64_t max_steps, int64_t check_every, double 
     done += n;
     ++k;
   }
+  // the last block's residual IS the residual of the returned state (its event has been waited for)
+  int* flag = reinterpret_cast<int*>(s->pinned + 6);
+  HR_CUDA(cudaMemcpyAsync(flag, s->plan.flag, sizeof(int), cudaMemcpyDeviceToHost, s->stream));
+  HR_CUDA(cudaStreamSynchronize(s->stream));
+  if (*flag) return fail(HR_ERR_NUMERIC, "psi_BL + u <= 0 or a non-finite value at an interior point");
   if (steps_done) *steps_done = done;
   if (n_history) *n_history = nh;
-  if (final_residual) {
-    double o3[3];
-    HR_TRY(hr_residual_ex(s, mode, o3));
-    *final_residual = o3[0];
-  } else {
-    HR_CUDA(cudaStreamSynchronize(s->stream));
-  }
+  if (final_residual) *final_residual = last_r;
   return HR_OK;
 }
 
@@ -727,6 +738,7 @@ hr_status hr_set_state(hr_solver* s, const void* u, const void* v, int32_t src_o
     HR_CUDA(hrk_unpack(s, s->a.Y[1], s->a.A[1]));
   }
   HR_CUDA(hrk_inner_fill(s, s->a.Y[0], s->a.Y[1]));
+  HR_CUDA(cudaMemsetAsync(s->plan.flag, 0, sizeof(int), s->stream));  // a new state: the numeric flag starts clear
   if (!src_on_device) HR_CUDA(cudaStreamSynchronize(s->stream));
   return HR_OK;
 }
@@ -834,6 +846,44 @@ hr_status hr_profile_step(hr_solver* s, int64_t n_steps, int32_t with_residual, 
     }
   }
   for (int i = 0; i < 6; ++i) ms6[i] = acc[i] / (double)n_steps;
+  return HR_OK;
+}
+
+hr_status hr_query(hr_solver* s, int32_t what, int64_t* value) {
+  if (!s || !value) return fail(HR_ERR_INVALID_ARG, "NULL argument");
+  switch (what) {
+    case HR_Q_STEP_GRAPH: *value = s->step_graph != nullptr; return HR_OK;
+    case HR_Q_RESID_GRAPH:
+      *value = (s->step_resid_graph[0] ? 1 : 0) | (s->step_resid_graph[1] ? 2 : 0);
+      return HR_OK;
+    case HR_Q_PERSISTENT: *value = 0; return HR_OK;
+    case HR_Q_NUMERIC_FLAG: {
+      int* flag = reinterpret_cast<int*>(s->pinned + 6);
+      HR_CUDA(cudaMemcpyAsync(flag, s->plan.flag, sizeof(int), cudaMemcpyDeviceToHost, s->stream));
+      HR_CUDA(cudaStreamSynchronize(s->stream));
+      *value = *flag;
+      return HR_OK;
+    }
+    case HR_Q_PLAN_ZC: *value = s->plan.zc; return HR_OK;
+    case HR_Q_PLAN_ITEMS: *value = (int64_t)s->plan.ntx * s->plan.nty * s->plan.nzc; return HR_OK;
+    case HR_Q_PLAN_GRID: *value = s->p.variant == 0 ? s->march_grid_lean[2] : s->march_grid[2]; return HR_OK;
+  }
+  return fail(HR_ERR_INVALID_ARG, "unknown query %d", what);
+}
+
+hr_status hr_measure_alu_peak(int32_t device, void* stream, int32_t dtype, int32_t packed, double* tflops) {
+  if (!tflops || (dtype != HR_F64 && dtype != HR_F32)) return fail(HR_ERR_INVALID_ARG, "bad arguments");
+  HR_CUDA(cudaSetDevice(device));
+  HR_CUDA(hrk_measure_alu(static_cast<cudaStream_t>(stream), dtype, packed, tflops));
+  return HR_OK;
+}
+
+hr_status hr_measure_launch_floor(int32_t device, void* stream, int32_t nodes, int32_t grid, int32_t block,
+                                  int32_t reps, double* us_per_graph) {
+  if (!us_per_graph || nodes < 1 || nodes > 64 || grid < 1 || block < 1 || block > 1024 || reps < 1 || !stream)
+    return fail(HR_ERR_INVALID_ARG, "need 1 <= nodes <= 64, grid >= 1, 1 <= block <= 1024, reps >= 1, a non-default stream");
+  HR_CUDA(cudaSetDevice(device));
+  HR_CUDA(hrk_measure_launch_floor(static_cast<cudaStream_t>(stream), nodes, grid, block, reps, us_per_graph));
   return HR_OK;
 }
 

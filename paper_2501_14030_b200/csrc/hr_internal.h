@@ -132,6 +132,7 @@ struct MarchPlan {
   int gt;        // tiles per group (whole tile rows); items are chunk-major within a group
   int* counters; // device: {next item, CTAs done} per stage kernel, zero between launches
   int sph;       // 1 = SinhSpherical inner map (theta -> pi - theta under rho -> -rho)
+  int* flag;     // device: set non-zero by a kernel that meets psi_BL + u <= 0 or NaN at an interior point
 };
 
 struct hr_solver {
@@ -160,6 +161,10 @@ struct hr_solver {
   int launches_per_step;
   void* workspace;
   size_t workspace_bytes;
+  // hr_relax: two pinned {num, den} slots and two events (the host tests block k-1 while block k runs),
+  // and the pinned word the numeric flag is read into; created once in hr_create
+  double* pinned = nullptr;
+  cudaEvent_t relax_ev[2] = {nullptr, nullptr};
 };
 
 // ---- hr_kernels.cu ----
@@ -191,3 +196,8 @@ MarchPlan hrk_make_plan(const int32_t n[3], int ng, int coord, int dtype);
 cudaError_t hrk_prepare(hr_solver* s);
 int hrk_max_partials(const int32_t n[3], int ng, int dtype);
 int hrk_launches_per_substep(const hr_solver* s);
+
+// ---- hr_measure.cu ----
+cudaError_t hrk_measure_alu(cudaStream_t st, int dtype, int packed, double* tflops);
+cudaError_t hrk_measure_launch_floor(cudaStream_t st, int nodes, int grid, int block, int reps,
+                                     double* us_per_graph);

@@ -652,6 +652,8 @@ static void choose_chunks(MarchPlan& m, int n2, int ng, int slots, bool f64) {
     // (config 3: +1.5 %, 512x256x256: +3 %; on 128^3 8 planes stay ahead)
     if (f64 && ntiles * ((n2 + 11) / 12) >= 4LL * slots) zc = 12;
     while (zc > 2 && ntiles * ((n2 + zc - 1) / zc) < slots) --zc;
+    // one plane per item where even that fits one wave of CTAs (config 0: the plane loop is a latency chain)
+    if (zc == 2 && ntiles * n2 <= slots) zc = 1;
   }
   if (zc > n2) zc = n2;
   m.nzc = (n2 + zc - 1) / zc;
@@ -913,9 +915,9 @@ cudaError_t hrk_prepare(hr_solver* s) {
 int hrk_max_partials(const int32_t n[3], int ng, int dtype) {
   (void)ng;
   const int direct = ((n[0] + RBX - 1) / RBX) * ((n[1] + RBY - 1) / RBY) * n[2];
-  // marching kernels: one partial pair per work item, chunks are at least 2 planes (or all of n2)
+  // marching kernels: one partial pair per work item; a work item has at least one plane
   const MarchPlan m = hrk_make_plan(n, ng, 0, dtype);
-  const long long march = (long long)m.ntx * m.nty * (n[2] / 2 + 1);
+  const long long march = (long long)m.ntx * m.nty * n[2];
   return direct > march ? direct : (int)march;
 }
 

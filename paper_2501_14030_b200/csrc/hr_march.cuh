@@ -168,11 +168,29 @@ __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(bar), "r"(bytes)
                : "memory");
 }
+// A lost TMA transaction must fail loudly, not hang -- but a long stall (compute-sanitizer, a debugger,
+// time-slicing, an ncu replay) is not a lost transaction: the watchdog is wall-clock based
+// (HR_MBAR_TIMEOUT_NS of %globaltimer, default 20 s; 0 compiles it out), looked at every 4096 failed polls.
+#ifndef HR_MBAR_TIMEOUT_NS
+#define HR_MBAR_TIMEOUT_NS 20000000000ull
+#endif
+__device__ __forceinline__ unsigned long long global_timer_ns() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
+}
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t phase) {
   uint32_t ok;
-  uint32_t spins = 0;
+  [[maybe_unused]] uint32_t spins = 0;
+  [[maybe_unused]] unsigned long long t0 = 0;
   do {
-    if (++spins > (1u << 24)) __trap();  // a lost TMA transaction must fail loudly, not hang
+#if HR_MBAR_TIMEOUT_NS
+    if ((++spins & 4095u) == 0) {
+      const unsigned long long now = global_timer_ns();
+      if (t0 == 0) t0 = now;
+      else if (now - t0 > HR_MBAR_TIMEOUT_NS) __trap();
+    }
+#endif
     asm volatile(
         "{\n.reg .pred p;\n"
         "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
@@ -427,8 +445,12 @@ __global__ void __launch_bounds__((TW / VX) * BY,
   // work items = (chunk of planes, tile), chunk-major
   const int ntiles = plan.ntx * plan.nty;
   const int n_items = ntiles * plan.nzc;
+  // no more items than CTAs (small grids): every CTA has exactly one item, nothing is handed out, and
+  // no atomic round trip sits at the end of the CTA's (short) life
+  const bool dynamic = n_items > (int)gridDim.x;
 
   double num = 0.0, den = 0.0;
+  bool bad = false;  // psi_BL + u <= 0 or NaN met at an interior point (the device flag)
   // ring position of the next plane to consume, and the parity its mbarrier completes with
   int sl = 0;
   uint32_t par = 0;
@@ -437,6 +459,53 @@ __global__ void __launch_bounds__((TW / VX) * BY,
   const uint64_t pol_keep = l2_policy_evict_last(), pol_stream = l2_policy_evict_first();
 #endif
 
+  // ---------------- outer points: radiation condition (a2, C13) + RK combine ----------------
+  // A grid-stride loop over the NG n1 n2 outer points, run by every CTA right after it has issued the
+  // first TMA loads of its first item, so that its load latency hides behind theirs (on L2-resident
+  // grids a CTA lives for one short item: anything serial at its end is on the critical path).
+  [[maybe_unused]] auto outer_tail = [&]() {
+    const int n_outer = NG * g.n1 * g.n2;
+    for (int m = blockIdx.x * NT + tid; m < n_outer; m += gridDim.x * NT) {
+      const int j = m % NG;
+      const int r = m / NG;
+      const int i1 = NG + r % g.n1, i2 = NG + r / g.n1;
+      const int i0 = g.n0 + NG + j;
+      const int c = g.off0 + i0 + g.P0 * i1 + s2 * i2;
+      const int qo = j + NG * i1;
+      const T r0 = a.RAD0[qo], r1 = a.RAD1[qo], ri = a.RADI[qo];
+      const T uc = a.in_u[c], vc = a.in_v[c];
+      const T ku = radiation_k(a.in_u, c, g.P0, r0, r1, ri);
+      const T kv = radiation_k(a.in_v, c, g.P0, r0, r1, ri);
+      T wu, wv;
+      if constexpr (LEAN) {
+        T yu = T(0), yv = T(0);
+        if constexpr (NEED_Y) { yu = a.y_u[c]; yv = a.y_v[c]; }  // lean stage 4: y_u / y_v point at Q
+        if constexpr (PREC && RK == 4) {  // Qd from the ACC buffer, Y through y_u / y_v
+          wu = rk_prec_4<T>(a.dt, ku, uc, a.acc_u[c], yu);
+          wv = rk_prec_4<T>(a.dt, kv, vc, a.acc_v[c], yv);
+        } else {
+          wu = rk_lean<T, RK>(a.dt, ku, uc, yu);
+          wv = rk_lean<T, RK>(a.dt, kv, vc, yv);
+        }
+        a.out_u[c] = wu;
+        a.out_v[c] = wv;
+        if constexpr (RK == 2 && PREC) {
+          a.acc_u[c] = rk_prec_q<T>(a.dt, ku, uc, yu);
+          a.acc_v[c] = rk_prec_q<T>(a.dt, kv, vc, yv);
+        } else if constexpr (RK == 2) {
+          a.acc_u[c] = (uc - yu) + (wu + wu);
+          a.acc_v[c] = (vc - yv) + (wv + wv);
+        }
+      } else {
+        rk_combine<T, RK>(a, c, ku, kv, uc, vc, wu, wv);
+      }
+      const int cB = i1 < 2 * NG ? 2 * NG - 1 - i1 : -1;
+      const int cC = i1 >= g.n1 ? 2 * (g.n1 + NG) - 1 - i1 : -1;
+      if (cB >= 0 || cC >= 0 || i2 < 2 * NG || i2 >= g.n2)
+        scatter_images<T>(ig, a.out_u, a.out_v, wu, wv, i0, i1, i2, -1, cB, cC);
+    }
+  };
+  [[maybe_unused]] bool tail_done = false;
   // The first item of a CTA is its block index; further items are handed out by an atomic counter
   // (items differ in cost: boundary tiles also write ghost images), except for the residual,
   // whose per-CTA partial sums must not depend on timing (C16: fixed reduction order).
@@ -491,6 +560,12 @@ __global__ void __launch_bounds__((TW / VX) * BY,
       for (int d = 0; d < D; ++d) {
         if (z_begin + d < z_end) issue(z_begin + d, sd);
         if (++sd == RING) sd = 0;
+      }
+    }
+    if constexpr (ADVANCE) {
+      if (!tail_done) {
+        outer_tail();
+        tail_done = true;
       }
     }
 
@@ -621,6 +696,7 @@ __global__ void __launch_bounds__((TW / VX) * BY,
             const F2 x = f2_add(L2(sb + ST_PSI * (TW * BY) + so), uc2);
             float x0, x1, r0, r1;
             f2_unpack(x, x0, x1);
+            bad |= !(x0 > 0.f) | (nact == VX & !(x1 > 0.f));
             asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r0) : "f"(x0));
             asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r1) : "f"(x1));
             F2 rr = f2_pack(r0, r1);
@@ -660,7 +736,9 @@ __global__ void __launch_bounds__((TW / VX) * BY,
           for (int j = 0; j < VX; ++j) {
             const T lap = l00[j] * d00[j] + l11[j] * d11[j] + l22[j] * d22[j] + l0[j] * d0[j] +
                           l1[j] * d1[j];
-            H[j] = lap + Ss.v[j] * pow_m7(psi.v[j] + HR_W(NG)[j]);
+            const T x = psi.v[j] + HR_W(NG)[j];
+            bad |= j < nact & !(x > T(0));
+            H[j] = lap + Ss.v[j] * pow_m7(x);
           }
           }
           if constexpr (RESID) {
@@ -790,6 +868,7 @@ __global__ void __launch_bounds__((TW / VX) * BY,
           for (int j = 0; j < WJ; ++j) p[k][j] = p[k + UR][j];
       }
     }
+    if (bad) *plan.flag = 1;
     if constexpr (RESID) {
       // one partial pair per ITEM, summed in a fixed order (thread: planes in order; then lanes,
       // then warps), so the result does not depend on which CTA ran the item or when (C16)
@@ -820,6 +899,7 @@ __global__ void __launch_bounds__((TW / VX) * BY,
       __syncthreads();  // red is reused by the next item
       item += gridDim.x;
     } else {
+      if (!dynamic) break;
       __syncthreads();  // all threads are done with this item (and with s_item, red)
       if (tid == 0) s_item = (int)gridDim.x + atomicAdd(plan.counters + 2 * STAGE, 1);
       __syncthreads();
@@ -830,7 +910,7 @@ __global__ void __launch_bounds__((TW / VX) * BY,
   // and, for the residual stages, sums the item partials in a fixed order (thread t takes items
   // t, t + NT, ...; then a fixed tree), so the reduction needs no launch of its own and its
   // result does not depend on which CTA happens to be last (C16).
-  if constexpr (ST != 5 || RESID) {
+  if (RESID || (ST != 5 && dynamic)) {
     __shared__ int s_last;
     if (tid == 0) {
       if constexpr (RESID) __threadfence();  // this CTA's partials before its "done" tick
@@ -883,47 +963,5 @@ __global__ void __launch_bounds__((TW / VX) * BY,
     }
   }
 
-  if constexpr (ADVANCE) {
-    // ---------------- outer points: radiation condition (a2, C13) + RK combine ----------------
-    const int n_outer = NG * g.n1 * g.n2;
-    for (int m = blockIdx.x * NT + tid; m < n_outer; m += gridDim.x * NT) {
-      const int j = m % NG;
-      const int r = m / NG;
-      const int i1 = NG + r % g.n1, i2 = NG + r / g.n1;
-      const int i0 = g.n0 + NG + j;
-      const int c = g.off0 + i0 + g.P0 * i1 + s2 * i2;
-      const int qo = j + NG * i1;
-      const T r0 = a.RAD0[qo], r1 = a.RAD1[qo], ri = a.RADI[qo];
-      const T uc = a.in_u[c], vc = a.in_v[c];
-      const T ku = radiation_k(a.in_u, c, g.P0, r0, r1, ri);
-      const T kv = radiation_k(a.in_v, c, g.P0, r0, r1, ri);
-      T wu, wv;
-      if constexpr (LEAN) {
-        T yu = T(0), yv = T(0);
-        if constexpr (NEED_Y) { yu = a.y_u[c]; yv = a.y_v[c]; }  // lean stage 4: y_u / y_v point at Q
-        if constexpr (PREC && RK == 4) {  // Qd from the ACC buffer, Y through y_u / y_v
-          wu = rk_prec_4<T>(a.dt, ku, uc, a.acc_u[c], yu);
-          wv = rk_prec_4<T>(a.dt, kv, vc, a.acc_v[c], yv);
-        } else {
-          wu = rk_lean<T, RK>(a.dt, ku, uc, yu);
-          wv = rk_lean<T, RK>(a.dt, kv, vc, yv);
-        }
-        a.out_u[c] = wu;
-        a.out_v[c] = wv;
-        if constexpr (RK == 2 && PREC) {
-          a.acc_u[c] = rk_prec_q<T>(a.dt, ku, uc, yu);
-          a.acc_v[c] = rk_prec_q<T>(a.dt, kv, vc, yv);
-        } else if constexpr (RK == 2) {
-          a.acc_u[c] = (uc - yu) + (wu + wu);
-          a.acc_v[c] = (vc - yv) + (wv + wv);
-        }
-      } else {
-        rk_combine<T, RK>(a, c, ku, kv, uc, vc, wu, wv);
-      }
-      const int cB = i1 < 2 * NG ? 2 * NG - 1 - i1 : -1;
-      const int cC = i1 >= g.n1 ? 2 * (g.n1 + NG) - 1 - i1 : -1;
-      if (cB >= 0 || cC >= 0 || i2 < 2 * NG || i2 >= g.n2)
-        scatter_images<T>(ig, a.out_u, a.out_v, wu, wv, i0, i1, i2, -1, cB, cC);
-    }
-  }
+
 }
