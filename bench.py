@@ -148,10 +148,29 @@ def cpu_baseline(p: dict, name: str) -> dict:
     n = max(1, min(50, int(12.0 / max(times[0], 1e-3))))
     times, o, threads = oracle_step_seconds(p, 1, n)
     per = float(np.mean(times))
-    return {"value": o.n_int * 4 / per, "unit": UNIT, "cores": threads, "kind": "oracle",
-            "sample": f"{n} x (residual + 1 RK4 step) of {name} in fp64 on the full grid, "
-                      f"{per:.3f} s each, u = v = 0 start; total incl. oracle set-up "
-                      f"{time.perf_counter() - t0:.1f} s"}
+    out = {"value": o.n_int * 4 / per, "unit": UNIT, "cores": threads, "kind": "oracle",
+           "sample": f"{n} x (residual + 1 RK4 step) of {name} in fp64 on the full grid, "
+                     f"{per:.3f} s each, u = v = 0 start; total incl. oracle set-up "
+                     f"{time.perf_counter() - t0:.1f} s"}
+    # the single-thread figure SURVEY.md section 8(d) asks for beside the all-cores one: the same oracle in a child
+    # process with OMP_NUM_THREADS=1, one warm-up + 2 timed (residual + RK4 step) on the same grid
+    try:
+        env = dict(os.environ, OMP_NUM_THREADS="1")
+        r = subprocess.run([sys.executable, os.path.abspath(__file__), "--oracle-single", "--workload", name],
+                           env=env, capture_output=True, text=True, timeout=600)
+        single = json.loads(r.stdout.strip().splitlines()[-1])
+        out["single_thread"] = {"value": single["value"], "unit": UNIT, "cores": single["cores"],
+                                "sample": single["sample"]}
+    except Exception as e:  # the all-cores figure stands on its own
+        out["single_thread"] = {"unavailable": repr(e)[:200]}
+    return out
+
+
+def oracle_single(p: dict, name: str):
+    times, o, threads = oracle_step_seconds(p, 1, 3)
+    per = float(np.mean(times[1:]))
+    print(json.dumps({"value": o.n_int * 4 / per, "cores": threads,
+                      "sample": f"2 x (residual + 1 RK4 step) of {name}, fp64, full grid, {per:.3f} s each"}))
 
 
 def run_reference(args, p, name):
@@ -207,8 +226,12 @@ def replicas_value(world: int, n_int: int, steps: int, sec_max: float) -> float:
 # ------------------------------------------------------------------------------------------------
 # the CUDA path
 # ------------------------------------------------------------------------------------------------
-def time_resident(torch, hr, p, dtype, steps, warmup, dist, flush_l2):
-    """K timed steps with the state resident in HBM; returns (seconds max over ranks, solver)."""
+MIN_TIMED_MS = 200.0  # the K-step block is repeated R times inside one event pair until the region is this long
+
+
+def time_resident(torch, hr, p, dtype, steps, warmup, dist, flush_l2, min_ms=MIN_TIMED_MS):
+    """K timed steps (x R repeats) with the state resident in HBM.
+    Returns (seconds per K steps, max over ranks; solver; R)."""
     s = hr.Solver(p, dtype=dtype, residual_mode=0)
     out2 = torch.zeros(2, dtype=torch.float64, device=s.device)
     flush = None
@@ -218,24 +241,40 @@ def time_resident(torch, hr, p, dtype, steps, warmup, dist, flush_l2):
     def one():
         s.hr_step_residual_async(0, out2)  # residual of the state + one RK4 step (Alg. 1 l.9-16)
 
+    def block(n):
+        e0 = torch.cuda.Event(enable_timing=True)
+        e1 = torch.cuda.Event(enable_timing=True)
+        e0.record(s.stream)
+        for _ in range(n):
+            one()
+        e1.record(s.stream)
+        e1.synchronize()
+        return e0.elapsed_time(e1)
+
     for _ in range(warmup):
         one()
     s.synchronize()
     torch.cuda.synchronize()
+    repeats = 1
+    burst_ms = None
+    if flush is None:
+        # calibrate R on a first block of K steps so that the timed region is >= min_ms (same R on every rank);
+        # that block, a few ms right after warm-up, is also the BURST figure: on B200 this kernel set slows by
+        # 10-15 % after ~50 ms of back-to-back steps (sw_power_cap: the SM clock drops and the plane loop is
+        # bound by SM latency, not by DRAM; a plain copy keeps 6.6 TB/s), so both are reported
+        cal = block(steps)
+        burst_ms = cal / steps
+        repeats = max(1, int(np.ceil(min_ms / max(cal, 1e-3))))
+        if dist is not None:
+            t = torch.tensor([repeats], dtype=torch.int64, device=s.device)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            repeats = int(t.item())
     if dist is not None:
         dist.barrier()
     torch.cuda.synchronize()
     if flush is None:
-        e0 = torch.cuda.Event(enable_timing=True)
-        e1 = torch.cuda.Event(enable_timing=True)
-        e0.record(s.stream)
-        for _ in range(steps):
-            one()
-        e1.record(s.stream)
-        e1.synchronize()
-        ms = e0.elapsed_time(e1)
+        ms = block(steps * repeats) / repeats
     else:  # L2-resident workload: flush between timed steps, time each step by its own event pair
-        ms = 0.0
         evs = []
         for _ in range(steps):
             with torch.cuda.stream(s.stream):
@@ -253,7 +292,25 @@ def time_resident(torch, hr, p, dtype, steps, warmup, dist, flush_l2):
     sec = max_over_ranks(torch, sec, dist, s.device)
     if dist is not None:
         dist.barrier()
-    return sec, s
+    s.burst_ms_per_step = burst_ms
+    return sec, s, repeats
+
+
+def time_warm(torch, s, steps):
+    """The same step back to back with nothing flushed in between (what hr_step(n) / hr_relax see on an
+    L2-resident grid); seconds per step."""
+    out2 = torch.zeros(2, dtype=torch.float64, device=s.device)
+    for _ in range(5):
+        s.hr_step_residual_async(0, out2)
+    s.synchronize()
+    e0 = torch.cuda.Event(enable_timing=True)
+    e1 = torch.cuda.Event(enable_timing=True)
+    e0.record(s.stream)
+    for _ in range(steps):
+        s.hr_step_residual_async(0, out2)
+    e1.record(s.stream)
+    e1.synchronize()
+    return e0.elapsed_time(e1) * 1e-3 / steps
 
 
 def time_e2e(torch, s, steps, warmup, dist):
@@ -288,27 +345,50 @@ def time_e2e(torch, s, steps, warmup, dist):
     return sec, 2 * s.ntot * w, 16
 
 
-def roofline(s, prof_ms, peak, peak_src):
-    """Fused substep kernel.  `achieved` follows SURVEY.md section 8(d): 10 w algorithmic bytes per interior
-    point-substep (8w, 12w, 12w, 8w for the stages of a running-sum RK4) x N_int points
-    per launch / mean launch duration.  The default arrangement forms the same RK4 step without the running
-    sum and moves 8 w per point-substep (6w, 10w, 8w, 8w); `moved_model_*` restates the fraction with
-    that count, `traffic` is the measured DRAM bytes per launch (ncu), so nothing hides behind the definition."""
+NOMINAL_HBM_GBS = 8000.0  # DGX B200 figure (7.7 TB/s HGX), context only (B200_PROFILING.md)
+
+
+def flops_per_point(fd_order: int) -> int:
+    """Algorithmic flops per interior point-substep: three second derivatives at
+    3n + 1 and two first derivatives at 3n - 1 flops (n = NG, symmetric pairing), ~10 for the metric
+    combination, ~25 for (psi + u)^-7 incl. one reciprocal, ~10 for k_u, c^2 and the RK combine."""
+    n = fd_order // 2
+    return 3 * (3 * n + 1) + 2 * (3 * n - 1) + 45
+
+
+def roofline(s, prof_ms, peak, peak_src, fd_order, traffic, alu_peak):
+    """Fused substep kernel, mean of the four stage launches.
+      achieved / frac     SURVEY.md section 8(d): 10 w algorithmic bytes per interior point-substep (running-sum RK4:
+                          8w, 12w, 12w, 8w) x N_int / mean launch duration -- kept so that rounds stay comparable
+      moved / frac_moved  the bytes the shipped arrangement has to move: 8 w per point-substep in fp64 (ACC-free
+                          RK4: 6w, 10w, 8w, 8w), 8.5 w in fp32 (its stage 4 also reads Y) -- THE distance to the roof
+      traffic / frac_dram DRAM bytes per launch ncu measured on the committed capture (profiles/traffic.json)
+      frac_nominal        moved bytes against the nominal 8 TB/s
+      alu                 algorithmic flops per second against the FMA peak measured in this
+                          run by hr_measure_alu_peak: shows which roof binds (HBM, by an order of magnitude)"""
     w = 8 if s.dtype == "f64" else 4
     mean_ms = sum(prof_ms[:4]) / 4.0
+    sec = mean_ms * 1e-3
     bytes_per_launch = 10 * w * s.n_int
-    moved = 8.0 * w * s.n_int
-    achieved = bytes_per_launch / (mean_ms * 1e-3) / 1e9
-    return {"bound": "hbm", "kernel": "fused substep k_march (RHS + radiation + RK combine + ghost images; stage 1 also "
+    moved = (8.0 if s.dtype == "f64" else 8.5) * w * s.n_int
+    achieved = bytes_per_launch / sec / 1e9
+    fl = flops_per_point(fd_order)
+    out = {"bound": "hbm", "kernel": "fused substep k_march (RHS + radiation + RK combine + ghost images; stage 1 also "
                                       "reduces the residual), mean of the 4 stages",
-            "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-            "peak_source": peak_src, "algorithmic_bytes_per_launch": bytes_per_launch,
-            "moved_model_bytes_per_launch": moved,
-            "moved_model_frac": moved / (mean_ms * 1e-3) / 1e9 / peak,
-            "launch_ms": {"stage1": prof_ms[0], "stage2": prof_ms[1], "stage3": prof_ms[2],
-                          "stage4": prof_ms[3], "inner_fill_x4": prof_ms[4], "residual": prof_ms[5]},
-            "substep_kernel_share_of_step": sum(prof_ms[:4]) / sum(prof_ms),
-            "traffic": None}
+           "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+           "peak_source": peak_src, "algorithmic_bytes_per_launch": bytes_per_launch,
+           "moved_bytes_per_launch": moved, "moved_GBs": moved / sec / 1e9, "frac_moved": moved / sec / 1e9 / peak,
+           "frac_nominal": moved / sec / 1e9 / NOMINAL_HBM_GBS, "peak_nominal": NOMINAL_HBM_GBS,
+           "traffic": traffic, "frac_dram": (traffic / sec / 1e9 / peak) if traffic else None,
+           "launch_ms": {"stage1": prof_ms[0], "stage2": prof_ms[1], "stage3": prof_ms[2],
+                         "stage4": prof_ms[3], "inner_fill_x4": prof_ms[4], "residual": prof_ms[5]},
+           "substep_kernel_share_of_step": sum(prof_ms[:4]) / sum(prof_ms),
+           "alu": {"flops_per_point_substep": fl, "achieved_tflops": fl * s.n_int / sec / 1e12,
+                   "peak_tflops": alu_peak, "frac": (fl * s.n_int / sec / 1e12 / alu_peak) if alu_peak else None,
+                   "peak_source": "measured in this run (hr_measure_alu_peak: register-resident FMA chains)",
+                   "arithmetic_intensity_flop_per_byte": fl / (moved / s.n_int),
+                   "ridge_flop_per_byte": (alu_peak * 1e3 / peak) if alu_peak else None}}
+    return out
 
 
 def load_peak():
@@ -338,8 +418,9 @@ def main():
     ap.add_argument("--workload", default="config3")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--oracle-single", action="store_true", help=argparse.SUPPRESS)
     ap.add_argument("--no-f32", action="store_true")
-    ap.add_argument("--no-also", action="store_true", help="skip the extra config1/config2 timings")
+    ap.add_argument("--no-also", action="store_true", help="skip the extra config0/1/2 timings")
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"],
                     help="precision of the headline leg (f32: for profiling the fp32 kernels alone)")
     args = ap.parse_args()
@@ -348,6 +429,9 @@ def main():
     name = args.workload
     p = workload(name)
 
+    if args.oracle_single:
+        oracle_single(p, name)
+        return
     if args.impl == "reference":
         run_reference(args, p, name)
         return
@@ -377,13 +461,25 @@ def main():
     if args.dtype == "f32":
         args.no_f32 = True
         flush_l2 = 10 * ntot * 4 <= 126e6
-    sec64, s64 = time_resident(torch, hr, p, args.dtype, args.steps, args.warmup, dist, flush_l2)
+    alu = {"f64": hr.hr_measure_alu_peak("f64", False, local),
+           "f32": max(hr.hr_measure_alu_peak("f32", False, local), hr.hr_measure_alu_peak("f32", True, local))}
+    sec64, s64, repeats = time_resident(torch, hr, p, args.dtype, args.steps, args.warmup, dist, flush_l2)
     launches_per_step = s64.launches_per_step  # the residual rides on the first substep's launch
     value = replicas_value(world, n_int, args.steps, sec64)
+    burst = None
+    if s64.burst_ms_per_step:
+        w64 = 8 if args.dtype == "f64" else 4
+        mv = (8.0 if args.dtype == "f64" else 8.5) * w64 * n_int * 4
+        burst = {"what": f"the first {args.steps} steps after warm-up, timed alone ({s64.burst_ms_per_step * args.steps:.1f} ms): "
+                         "before the power cap lowers the SM clock; `value` is the sustained figure",
+                 "value": world * n_int * 4 / (s64.burst_ms_per_step * 1e-3), "ms_per_step": s64.burst_ms_per_step,
+                 "frac_moved": mv / (s64.burst_ms_per_step * 1e-3) / 1e9 / peak}
+    path = {"step_graph": s64.hr_query("step_graph"), "resid_graph": s64.hr_query("resid_graph"),
+            "plan_zc": s64.hr_query("plan_zc"), "plan_items": s64.hr_query("plan_items"),
+            "plan_grid": s64.hr_query("plan_grid")}
 
-    prof64 = s64.hr_profile_step(min(args.steps, 20), True)
-    roof = roofline(s64, prof64, peak, peak_src)
-    roof["traffic"] = load_traffic(args.dtype)
+    prof64 = s64.hr_profile_step(min(max(args.steps, 20), 100), True)
+    roof = roofline(s64, prof64, peak, peak_src, p["fd_order"], load_traffic(args.dtype), alu[args.dtype])
     sec_e2e, h2d, d2h = time_e2e(torch, s64, max(3, min(args.steps, 10)), 3, dist)
     e2e_steps = max(3, min(args.steps, 10))
     e2e = {"value": world * n_int * 4 * e2e_steps / sec_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d,
@@ -396,13 +492,14 @@ def main():
 
     f32 = None
     if not args.no_f32:
-        sec32, s32 = time_resident(torch, hr, p, "f32", args.steps, args.warmup, dist,
-                                   10 * ntot * 4 <= 126e6)
-        prof32 = s32.hr_profile_step(min(args.steps, 20), True)
-        r32 = roofline(s32, prof32, peak, peak_src)
-        r32["traffic"] = load_traffic("f32")
+        sec32, s32, rep32 = time_resident(torch, hr, p, "f32", args.steps, args.warmup, dist,
+                                          10 * ntot * 4 <= 126e6)
+        prof32 = s32.hr_profile_step(min(max(args.steps, 20), 100), True)
+        r32 = roofline(s32, prof32, peak, peak_src, p["fd_order"], load_traffic("f32"), alu["f32"])
         f32 = {"value": world * n_int * 4 * args.steps / sec32, "unit": UNIT,
-               "ms_per_step": 1e3 * sec32 / args.steps, "roofline": r32}
+               "ms_per_step": 1e3 * sec32 / args.steps, "repeats": rep32, "roofline": r32,
+               "burst": {"value": world * n_int * 4 / (s32.burst_ms_per_step * 1e-3),
+                         "ms_per_step": s32.burst_ms_per_step} if s32.burst_ms_per_step else None}
         s32.close()
         del s32
 
@@ -415,7 +512,7 @@ def main():
     also = None
     if world == 1 and args.workload == "config3" and not args.no_also:
         also = {}
-        for other in ("config1", "config2"):
+        for other in ("config0", "config1", "config2"):
             po = workload(other)
             To = [x + po["fd_order"] for x in po["n"]]
             nto = To[0] * To[1] * To[2]
@@ -423,8 +520,20 @@ def main():
             entry = {"n_interior": list(po["n"]), "fd_order": po["fd_order"],
                      "l2": "L2 flushed between timed steps" if 10 * nto * 8 <= 126e6 else "larger than L2"}
             for dt, w in (("f64", 8), ("f32", 4)):
-                sec, so = time_resident(torch, hr, po, dt, 20, 3, None, 10 * nto * w <= 126e6)
-                entry[dt] = {"value": nio * 4 * 20 / sec, "unit": UNIT, "ms_per_step": 1e3 * sec / 20}
+                sec, so, _ = time_resident(torch, hr, po, dt, 50, 5, None, 10 * nto * w <= 126e6)
+                warm = time_warm(torch, so, 200)
+                grid = so.hr_query("plan_grid")
+                # the floor under a step of 4 dependent launches of this grid, whatever the kernels do
+                floor_us = hr.hr_measure_launch_floor(4, int(grid), 128, 300, local)
+                moved_w = 8.0 if dt == "f64" else 8.5
+                entry[dt] = {"value": nio * 4 * 50 / sec, "unit": UNIT, "ms_per_step": 1e3 * sec / 50,
+                             "warm_l2": {"value": nio * 4 / warm, "ms_per_step": 1e3 * warm,
+                                         "what": "steps back to back, nothing flushed (hr_step(n), hr_relax)"},
+                             "launch_floor_ms_per_step": 1e-3 * floor_us,
+                             "floor_what": f"CUDA graph of 4 dependent empty launches, {grid} CTAs x 128 threads",
+                             "frac_moved_warm": moved_w * w * nio * 4 / warm / 1e9 / peak,
+                             "plan": {"zc": so.hr_query("plan_zc"), "items": so.hr_query("plan_items"),
+                                      "grid": grid}}
                 so.close()
                 del so
             also[other] = entry
@@ -440,7 +549,8 @@ def main():
             "warmup": args.warmup, "ms_per_step": 1e3 * sec64 / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
             "config": config_dict(p, name, world), "clocks": clocks, "e2e": e2e,
-            "gpu_launches": launches_per_step * args.steps, "roofline": roof, "f32": f32,
+            "gpu_launches": launches_per_step * args.steps * repeats, "repeats": repeats,
+            "timed_region_ms": 1e3 * sec64 * repeats, "burst": burst, "roofline": roof, "f32": f32, "path": path,
             "library": hr.hr_version()}
     if also is not None:
         line["also"] = also
