@@ -10,7 +10,9 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libhr_b200.so")
+# HR_B200_LIB=libhr_b200_nofmad.so selects the --fmad=false twin of the library (same sources, the ablation of
+# PAPER.md:193, 301-321; built by build.py next to the product library); a file name inside this directory only
+LIB_PATH = os.path.join(_HERE, os.path.basename(os.environ.get("HR_B200_LIB", "libhr_b200.so")))
 
 HR_OK = 0
 HR_SINHSPHERICAL, HR_SINHSYMTP = 0, 1

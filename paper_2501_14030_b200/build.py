@@ -10,7 +10,11 @@ LIB = os.path.join(HERE, "libhr_b200.so")
 SOURCES = ["hr_api.cu", "hr_kernels.cu", "hr_measure.cu"]
 HEADERS = ["hr_internal.h", "fd_tables.cuh", "hr_march.cuh", os.path.join(ROOT, "include", "hr.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-              "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--fmad=true"]
+              "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]
+# The ablation of PAPER.md:193, 301-321: the same sources with FMA contraction switched off
+# (plain expressions compile to separate multiplies and adds; the explicit fma() of the reciprocal's Newton
+# steps stays).  Loaded instead of the product library when HR_B200_LIB names it (binding.py).
+LIB_NOFMAD = os.path.join(HERE, "libhr_b200_nofmad.so")
 
 
 def _nvcc() -> str:
@@ -29,29 +33,40 @@ def _stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and not _stale():
-        return LIB
-    objs, procs = [], []
-    for src in SOURCES:  # the translation units compile side by side
-        obj = os.path.join(CSRC, src.replace(".cu", ".o"))
-        # HR_NVCC_DEFS="-DHR_MARCH_D_F64=3 ...": tuning overrides of the macros in hr_internal.h
-        cmd = [_nvcc(), *NVCC_FLAGS, *os.environ.get("HR_NVCC_DEFS", "").split(), "-c",
-               os.path.join(CSRC, src), "-o", obj]
-        if verbose:
-            cmd.insert(1, "-Xptxas=-v")
-        procs.append((cmd, subprocess.Popen(cmd)))
-        objs.append(obj)
+def _compile_all(jobs, verbose):
+    """jobs: (library path, object suffix, extra flags); every translation unit of every job side by side."""
+    procs = []
+    for lib, suffix, extra in jobs:
+        for src in SOURCES:
+            obj = os.path.join(CSRC, src.replace(".cu", suffix + ".o"))
+            # HR_NVCC_DEFS="-DHR_MARCH_D_F64=3 ...": tuning overrides of the macros in hr_internal.h
+            cmd = [_nvcc(), *NVCC_FLAGS, *extra, *os.environ.get("HR_NVCC_DEFS", "").split(), "-c",
+                   os.path.join(CSRC, src), "-o", obj]
+            if verbose:
+                cmd.insert(1, "-Xptxas=-v")
+            procs.append((cmd, subprocess.Popen(cmd)))
     for cmd, pr in procs:
         if pr.wait() != 0:
             raise subprocess.CalledProcessError(pr.returncode, cmd)
-    tmp = LIB + f".tmp{os.getpid()}"
-    subprocess.run([_nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", *objs,
-                    "-o", tmp], check=True)
-    os.replace(tmp, LIB)
+    for lib, suffix, _ in jobs:
+        objs = [os.path.join(CSRC, src.replace(".cu", suffix + ".o")) for src in SOURCES]
+        tmp = lib + f".tmp{os.getpid()}"
+        subprocess.run([_nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", *objs,
+                        "-o", tmp], check=True)
+        os.replace(tmp, lib)
+
+
+def build(force: bool = False, verbose: bool = False, ablation: bool = True) -> str:
+    """The product library (FMA contraction on, nvcc's default) and, with `ablation`, its --fmad=false twin."""
+    if not force and not _stale() and (not ablation or os.path.exists(LIB_NOFMAD)):
+        return LIB
+    jobs = [(LIB, "", ["--fmad=true"])]
+    if ablation:
+        jobs.append((LIB_NOFMAD, "_nofmad", ["--fmad=false"]))
+    _compile_all(jobs, verbose)
     return LIB
 
 
 if __name__ == "__main__":
     import sys
-    print(build(force=True, verbose="-v" in sys.argv))
+    print(build(force=True, verbose="-v" in sys.argv, ablation="--no-ablation" not in sys.argv))
