@@ -34,12 +34,14 @@
 extern "C" {
 #endif
 
-enum { ORC_SINHSPHERICAL = 0, ORC_SINHSYMTP = 1 };
+/* "Cartesian-like, spherical-like, cylindrical-like, and bispherical-like" reference metrics.
+ * 0, 1: readings C4; 2: reading C24. */
+enum { ORC_SINHSPHERICAL = 0, ORC_SINHSYMTP = 1, ORC_SINHCYLINDRICAL = 2 };
 
 /* One puncture = 10 doubles: m, pos[3], P[3], S[3] (Cartesian). */
 typedef struct {
   int32_t n[3];        /* interior points N0 N1 N2 (N2 even)                         */
-  int32_t coord;       /* ORC_SINHSPHERICAL | ORC_SINHSYMTP  (C4)                    */
+  int32_t coord;       /* ORC_SINHSPHERICAL | ORC_SINHSYMTP (C4) | ORC_SINHCYLINDRICAL (C24) */
   int32_t fd_order;    /* 2,4,...,12; NG = fd_order/2 (C7)             */
   int32_t n_punctures;
   double amp, sinhw;   /* AMPL/SINHW or AMAX/SINHWAA (C4, C5)                        */

@@ -12,6 +12,7 @@ from . import build as _build
 
 SINHSPHERICAL = 0
 SINHSYMTP = 1
+SINHCYLINDRICAL = 2
 
 _i32p = C.POINTER(C.c_int32)
 _f64p = C.POINTER(C.c_double)
@@ -122,7 +123,7 @@ class Oracle:
         self._punct = _punct_array(params["punctures"])
         p = _Params()
         p.n[:] = [int(x) for x in params["n"]]
-        p.coord = {"SinhSpherical": 0, "SinhSymTP": 1}[params["coord"]]
+        p.coord = {"SinhSpherical": 0, "SinhSymTP": 1, "SinhCylindrical": 2}[params["coord"]]
         p.fd_order = int(params["fd_order"])
         p.n_punctures = int(self._punct.shape[0])
         p.amp = float(params["amp"])

@@ -67,11 +67,22 @@ static void orc_rho(double amp, double W, double x0, double* r, double* rp, doub
 
 /* C4: (x0, x1 = theta, x2 = phi) -> Cartesian, grid-centred.
  *   SinhSpherical: (r sin th cos ph, r sin th sin ph, r cos th),            r = rho(x0)
- *   SinhSymTP:     (A sin th cos ph, A sin th sin ph, sqrt(A^2+b^2) cos th), A = rho(x0) */
+ *   SinhSymTP:     (A sin th cos ph, A sin th sin ph, sqrt(A^2+b^2) cos th), A = rho(x0)
+ * C24 ("cylindrical-like"): x0 in [0,1], x1 in [-1,1], x2 = phi in [-pi,pi);
+ *   SinhCylindrical: (R cos ph, R sin ph, Z),  R = rho(x0), Z = rho(x1)  (the same sinh map, same
+ *   amplitude and width, along the axis; the periodic coordinate is x2 as in the other systems)    */
 void orc_map_to_cart(int32_t coord, double amp, double sinhw, double bscale, double x0,
                      double x1, double x2, double* xyz) {
   double r, rp, rpp;
   orc_rho(amp, sinhw, x0, &r, &rp, &rpp);
+  if (coord == ORC_SINHCYLINDRICAL) {
+    double z, zp, zpp;
+    orc_rho(amp, sinhw, x1, &z, &zp, &zpp);
+    xyz[0] = r * cos(x2);
+    xyz[1] = r * sin(x2);
+    xyz[2] = z;
+    return;
+  }
   const double st = sin(x1), ct = cos(x1), sp = sin(x2), cp = cos(x2);
   xyz[0] = r * st * cp;
   xyz[1] = r * st * sp;
@@ -89,6 +100,14 @@ void orc_map_from_cart(int32_t coord, double amp, double sinhw, double bscale,
   const double rc2 = x * x + y * y; /* cylindrical radius squared */
   const double rc = sqrt(rc2);
   double rad, th;
+  if (coord == ORC_SINHCYLINDRICAL) { /* C24: x0 from the cylindrical radius, x1 from z, same sinh map */
+    double ph = atan2(y, x);
+    if (ph >= ORC_PI) ph -= 2.0 * ORC_PI;
+    x012[0] = sinhw * asinh(rc * sinh(1.0 / sinhw) / amp);
+    x012[1] = sinhw * asinh(z * sinh(1.0 / sinhw) / amp);
+    x012[2] = ph;
+    return;
+  }
   if (coord == ORC_SINHSPHERICAL) {
     rad = sqrt(rc2 + z * z);
     th = atan2(rc, z);
@@ -122,6 +141,21 @@ void orc_metric_at(int32_t coord, double amp, double sinhw, double bscale, doubl
                    double* h, double* gfac) {
   double r, rp, rpp;
   orc_rho(amp, sinhw, x0, &r, &rp, &rpp);
+  if (coord == ORC_SINHCYLINDRICAL) {
+    /* C24: h = (R', Z', R);  lap u = u_00/R'^2 + u_11/Z'^2 + u_22/R^2
+     *                                + [1/(R R') - R''/R'^3] u_0 - [Z''/Z'^3] u_1               */
+    double z, zp, zpp;
+    orc_rho(amp, sinhw, x1, &z, &zp, &zpp);
+    h[0] = rp;
+    h[1] = zp;
+    h[2] = r;
+    gfac[0] = 1.0 / (rp * rp);
+    gfac[1] = 1.0 / (zp * zp);
+    gfac[2] = 1.0 / (r * r);
+    gfac[3] = 1.0 / (r * rp) - rpp / (rp * rp * rp);
+    gfac[4] = -zpp / (zp * zp * zp);
+    return;
+  }
   const double st = sin(x1), ct = cos(x1);
   if (coord == ORC_SINHSPHERICAL) {
     h[0] = rp;
@@ -156,6 +190,15 @@ static void orc_radial_at(int32_t coord, double amp, double sinhw, double bscale
                           double x1, double* rad0, double* rad1, double* invr) {
   double r, rp, rpp;
   orc_rho(amp, sinhw, x0, &r, &rp, &rpp);
+  if (coord == ORC_SINHCYLINDRICAL) { /* C24: r^2 = R^2 + Z^2, d_r = (R/r) d_R + (Z/r) d_Z */
+    double z, zp, zpp;
+    orc_rho(amp, sinhw, x1, &z, &zp, &zpp);
+    const double dist = sqrt(r * r + z * z);
+    *rad0 = r / (dist * rp);
+    *rad1 = z / (dist * zp);
+    *invr = 1.0 / dist;
+    return;
+  }
   if (coord == ORC_SINHSPHERICAL) {
     *rad0 = 1.0 / rp;
     *rad1 = 0.0;
@@ -224,15 +267,28 @@ static int orc_is_interior(const orc_grid* g, int a, int i) {
 
 /* C14: nearest grid index of coordinate x along axis a, and the fractional error. */
 static int orc_nearest_index(const orc_grid* g, int a, double x, double* frac_err) {
-  const double xmin = (a == 2) ? -ORC_PI : 0.0;
+  const double xmin = (a == 2) ? -ORC_PI : ((a == 1 && g->p.coord == ORC_SINHCYLINDRICAL) ? -1.0 : 0.0);
   const double j = (x - xmin) / g->dx[a] - 0.5 + (double)g->ng;
   const double jr = floor(j + 0.5);
   *frac_err = fabs(j - jr);
   return (int)jr;
 }
 
+/* C13: is the ghost point (i0,i1,i2) an OUTER point (radiation condition) rather than an inner one?
+ *   SinhSpherical, SinhSymTP: i0 >= N0+NG with interior angles;
+ *   SinhCylindrical (C24): beyond the outer cylinder or beyond either end face, i.e. x0 >= 0 and
+ *   (i0 >= N0+NG or x1 outside [-1,1]), with interior phi.
+ * These are exactly the ghost points whose Cartesian image maps back to themselves (a point
+ * beyond the domain has no other representative); every other ghost point is an inner point. */
+static int orc_is_outer(const orc_grid* g, int i0, int i1, int i2) {
+  const int in1 = orc_is_interior(g, 1, i1), in2 = orc_is_interior(g, 2, i2);
+  if (!in2 || i0 < g->ng) return 0;
+  if (g->p.coord == ORC_SINHCYLINDRICAL) return (i0 >= g->p.n[0] + g->ng) || !in1;
+  return (i0 >= g->p.n[0] + g->ng) && in1;
+}
+
 /* PAPER.md:200 (Alg. 1 l.4), C13 + C14: classify every ghost point.
- *   outer : i0 >= N0+NG with interior angles (radiation condition is applied there);
+ *   outer : see orc_is_outer (the radiation condition is applied there);
  *   inner : every other ghost point; its Cartesian image mapped back into the fundamental
  *           domain lands on another grid point src, and value[dst] = +1 * value[src].      */
 static int orc_build_bc(orc_grid* g) {
@@ -244,7 +300,7 @@ static int orc_build_bc(orc_grid* g) {
         const int in0 = orc_is_interior(g, 0, i0), in1 = orc_is_interior(g, 1, i1),
                   in2 = orc_is_interior(g, 2, i2);
         if (in0 && in1 && in2) continue;
-        if (i0 >= g->p.n[0] + g->ng && in1 && in2)
+        if (orc_is_outer(g, i0, i1, i2))
           ++n_outer;
         else
           ++n_inner;
@@ -263,7 +319,7 @@ static int orc_build_bc(orc_grid* g) {
                   in2 = orc_is_interior(g, 2, i2);
         if (in0 && in1 && in2) continue;
         const int64_t idx = orc_idx(g, i0, i1, i2);
-        if (i0 >= g->p.n[0] + g->ng && in1 && in2) {
+        if (orc_is_outer(g, i0, i1, i2)) {
           g->outer_idx[ko++] = (int32_t)idx;
           continue;
         }
@@ -278,6 +334,7 @@ static int orc_build_bc(orc_grid* g) {
         }
         if (s[0] < 0 || s[0] >= T0 || s[1] < 0 || s[1] >= T1 || s[2] < 0 || s[2] >= T2)
           return -1;
+        if (s[0] == i0 && s[1] == i1 && s[2] == i2) return -1; /* an inner point has another representative */
         g->inner_dst[ki] = (int32_t)idx;
         g->inner_src[ki] = (int32_t)orc_idx(g, s[0], s[1], s[2]);
         ++ki;
@@ -289,7 +346,8 @@ static int orc_build_bc(orc_grid* g) {
 orc_grid* orc_create(const orc_params* p) {
   if (!p) return NULL;
   if (p->fd_order < 2 || p->fd_order > 2 * ORC_MAX_NG || (p->fd_order % 2)) return NULL;
-  if (p->coord != ORC_SINHSPHERICAL && p->coord != ORC_SINHSYMTP) return NULL;
+  if (p->coord != ORC_SINHSPHERICAL && p->coord != ORC_SINHSYMTP && p->coord != ORC_SINHCYLINDRICAL)
+    return NULL;
   const int ng = p->fd_order / 2;
   for (int a = 0; a < 3; ++a)
     if (p->n[a] < ng) return NULL;
@@ -314,15 +372,16 @@ orc_grid* orc_create(const orc_params* p) {
     return NULL;
   }
 
-  /* C8: cell-centred uniform coordinates, x0 in [0,1], x1 in [0,pi], x2 in [-pi,pi]. */
+  /* C8: cell-centred uniform coordinates, x0 in [0,1], x1 in [0,pi] (C24: [-1,1]), x2 in [-pi,pi]. */
+  const double x1min = (p->coord == ORC_SINHCYLINDRICAL) ? -1.0 : 0.0;
   g->dx[0] = 1.0 / (double)p->n[0];
-  g->dx[1] = ORC_PI / (double)p->n[1];
+  g->dx[1] = ((p->coord == ORC_SINHCYLINDRICAL) ? 2.0 : ORC_PI) / (double)p->n[1];
   g->dx[2] = 2.0 * ORC_PI / (double)p->n[2];
   g->x0 = (double*)malloc(sizeof(double) * (size_t)g->T[0]);
   g->x1 = (double*)malloc(sizeof(double) * (size_t)g->T[1]);
   g->x2 = (double*)malloc(sizeof(double) * (size_t)g->T[2]);
   for (int i = 0; i < g->T[0]; ++i) g->x0[i] = ((double)(i - ng) + 0.5) * g->dx[0];
-  for (int i = 0; i < g->T[1]; ++i) g->x1[i] = ((double)(i - ng) + 0.5) * g->dx[1];
+  for (int i = 0; i < g->T[1]; ++i) g->x1[i] = x1min + ((double)(i - ng) + 0.5) * g->dx[1];
   for (int i = 0; i < g->T[2]; ++i) g->x2[i] = -ORC_PI + ((double)(i - ng) + 0.5) * g->dx[2];
 
   orc_fd_weights(p->fd_order, g->c1, g->d2);

@@ -87,7 +87,10 @@ void FN(orc_rhs_interior)(const orc_grid* g, const real* u, const real* v, real*
 
 /* a2, C13: outgoing-radiation (Sommerfeld) condition at the outer points, applied to k:
  *   k_f = -c [ d_r f + (f - f_inf)/r ],  f_inf = 0,  f in {u, v};
- *   d_r f = rad0 d_0 f + rad1 d_1 f  with the 2nd-order backward d_0 and centred d_1.       */
+ *   d_r f = rad0 d_0 f + rad1 d_1 f,  each derivative 2nd order: one-sided, pointing into the grid,
+ *   along an axis in which the point lies beyond the interior (backward on the high side, forward
+ *   on the low side), centred otherwise.  SinhSpherical / SinhSymTP outer points lie beyond x0 only
+ *   (backward d_0, centred d_1); SinhCylindrical ones (C24) also beyond either end of x1.        */
 void FN(orc_bc_outer)(const orc_grid* g, const real* u, const real* v, real* ku, real* kv) {
   const int64_t s1 = g->T[0];
   const real h0 = (real)(1.0 / (2.0 * g->dx[0])), h1 = (real)(1.0 / (2.0 * g->dx[1]));
@@ -95,13 +98,25 @@ void FN(orc_bc_outer)(const orc_grid* g, const real* u, const real* v, real* ku,
   for (int64_t m = 0; m < g->n_outer; ++m) {
     const int64_t c = g->outer_idx[m];
     const size_t q = (size_t)(c % ((int64_t)g->T[0] * g->T[1]));
+    const int i0 = (int)(q % (size_t)g->T[0]), i1 = (int)(q / (size_t)g->T[0]);
+    const int hi0 = i0 >= g->p.n[0] + g->ng;
+    const int hi1 = i1 >= g->p.n[1] + g->ng, lo1 = i1 < g->ng;
     const real cw = (real)g->c[q], r0 = (real)g->rad0[q], r1 = (real)g->rad1[q],
                ir = (real)g->invr[q];
     const real* f[2] = {u, v};
     real* k[2] = {ku, kv};
     for (int a = 0; a < 2; ++a) {
-      const real d0 = ((real)3 * f[a][c] - (real)4 * f[a][c - 1] + f[a][c - 2]) * h0;
-      const real d1 = (f[a][c + s1] - f[a][c - s1]) * h1;
+      real d0, d1;
+      if (hi0)
+        d0 = ((real)3 * f[a][c] - (real)4 * f[a][c - 1] + f[a][c - 2]) * h0;
+      else
+        d0 = (f[a][c + 1] - f[a][c - 1]) * h0;
+      if (hi1)
+        d1 = ((real)3 * f[a][c] - (real)4 * f[a][c - s1] + f[a][c - 2 * s1]) * h1;
+      else if (lo1)
+        d1 = ((real)4 * f[a][c + s1] - (real)3 * f[a][c] - f[a][c + 2 * s1]) * h1;
+      else
+        d1 = (f[a][c + s1] - f[a][c - s1]) * h1;
       k[a][c] = -cw * (r0 * d0 + r1 * d1 + f[a][c] * ir);
     }
   }
