@@ -200,7 +200,7 @@ class Solver:
     dedicated torch stream (`self.stream`)."""
 
     def __init__(self, params: dict, dtype="f64", device=0, residual_mode=0, variant=0,
-                 stream=None):
+                 stream=None, poison=False):
         import torch  # device memory and streams only
 
         self._h = None
@@ -217,6 +217,8 @@ class Solver:
                                           residual_mode, variant)
         nbytes = hr_workspace_bytes(self.p)
         self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        if poison:  # every byte 0xFF = NaN in both precisions: a read of workspace the library never wrote shows
+            self.workspace.fill_(255)
         base = self.workspace.data_ptr()
         self._ws_ptr = (base + 255) // 256 * 256
         h = _vp()

@@ -5,12 +5,14 @@
 // hr_kernels.cu; there is no CPU fallback.  Product code: nothing here touches oracle/.
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
 #include <limits>
+#include <mutex>
 #include <new>
 
 #include "hr_internal.h"
@@ -352,6 +354,8 @@ hr_status enqueue_rk4_step(const hr_solver* s) {
   return HR_OK;
 }
 
+void forget_many_graphs(const hr_solver* s);  // hr_step_many's cached graphs, below
+
 }  // namespace
 
 extern "C" {
@@ -552,6 +556,7 @@ hr_status hr_host_setup(const hr_params* p, double* dt, double* dsmin, int64_t* 
 
 hr_status hr_destroy(hr_solver* s) {
   if (!s) return HR_OK;
+  forget_many_graphs(s);
   if (s->step_graph) cudaGraphExecDestroy(s->step_graph);
   for (cudaGraphExec_t g : s->step_resid_graph)
     if (g) cudaGraphExecDestroy(g);
@@ -603,11 +608,106 @@ hr_status hr_step_residual_async(hr_solver* s, int32_t mode, double* out2_dev) {
   return HR_OK;
 }
 
+// hr_step_many: the N solvers' steps as ONE CUDA graph with N parallel branches of k RK4 steps each (captured
+// once per solver set and k, cached).  On small grids a step is four ~6 us kernels that fill a fraction of the
+// SMs: replaying per-solver graphs from the host is bound by the host's launch rate (profiles/r1c.md: 1.5-1.7x
+// at N = 7), while one graph lets the device overlap the branches and costs one launch per k steps of all N.
+}  // extern "C"
+
+namespace {
+
+struct ManyGraph {
+  std::vector<hr_solver*> key;
+  int k;
+  cudaGraphExec_t exec;
+};
+std::mutex g_many_mu;
+std::vector<ManyGraph> g_many;
+constexpr int kManyStepsPerGraph = 8;
+
+cudaGraphExec_t many_graph(hr_solver* const* solvers, int32_t n, int k) {
+  std::lock_guard<std::mutex> lock(g_many_mu);
+  for (const ManyGraph& m : g_many)
+    if (m.k == k && (int32_t)m.key.size() == n && std::equal(m.key.begin(), m.key.end(), solvers)) return m.exec;
+  cudaStream_t s0 = solvers[0]->stream;
+  std::vector<cudaEvent_t> ev((size_t)n, nullptr);
+  bool ok = true;
+  for (auto& e : ev) ok = ok && cudaEventCreateWithFlags(&e, cudaEventDisableTiming) == cudaSuccess;
+  cudaGraph_t graph = nullptr;
+  cudaGraphExec_t exec = nullptr;
+  if (ok && cudaStreamBeginCapture(s0, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+    ok = cudaEventRecord(ev[0], s0) == cudaSuccess;  // fork
+    for (int32_t i = 1; i < n && ok; ++i)
+      if (solvers[i]->stream != s0) ok = cudaStreamWaitEvent(solvers[i]->stream, ev[0], 0) == cudaSuccess;
+    // the branches run side by side: each solver chunks its grid as if 1/n of the CTA slots were its own
+    // (longer chunks, fewer window primings; bit-identical results, the plan only orders the work)
+    for (int32_t i = 0; i < n; ++i) hrk_replan(solvers[i], n);
+    for (int32_t i = 0; i < n && ok; ++i)
+      for (int it = 0; it < k && ok; ++it) ok = enqueue_rk4_step(solvers[i]) == HR_OK;
+    for (int32_t i = 0; i < n; ++i) hrk_replan(solvers[i], 1);
+    for (int32_t i = 1; i < n && ok; ++i) {  // join
+      if (solvers[i]->stream == s0) continue;
+      ok = cudaEventRecord(ev[i], solvers[i]->stream) == cudaSuccess &&
+           cudaStreamWaitEvent(s0, ev[i], 0) == cudaSuccess;
+    }
+    const cudaError_t ce = cudaStreamEndCapture(s0, &graph);
+    if (!ok || ce != cudaSuccess || !graph || cudaGraphInstantiate(&exec, graph, 0) != cudaSuccess) exec = nullptr;
+    if (graph) cudaGraphDestroy(graph);
+  }
+  cudaGetLastError();
+  for (cudaEvent_t e : ev)
+    if (e) cudaEventDestroy(e);
+  if (exec) g_many.push_back(ManyGraph{std::vector<hr_solver*>(solvers, solvers + n), k, exec});
+  return exec;
+}
+
+void forget_many_graphs(const hr_solver* s) {  // hr_destroy: graphs that replay this solver's kernels
+  std::lock_guard<std::mutex> lock(g_many_mu);
+  for (size_t i = 0; i < g_many.size();) {
+    if (std::find(g_many[i].key.begin(), g_many[i].key.end(), s) != g_many[i].key.end()) {
+      cudaGraphExecDestroy(g_many[i].exec);
+      g_many.erase(g_many.begin() + (long)i);
+    } else {
+      ++i;
+    }
+  }
+}
+
+}  // namespace
+
+extern "C" {
+
 hr_status hr_step_many(hr_solver* const* solvers, int32_t n, int64_t n_steps) {
   if (n < 0 || n_steps < 0 || (n > 0 && !solvers)) return fail(HR_ERR_INVALID_ARG, "bad arguments");
   for (int32_t i = 0; i < n; ++i)
     if (!solvers[i]) return fail(HR_ERR_INVALID_ARG, "solver %d is NULL", i);
-  for (int64_t it = 0; it < n_steps; ++it)
+  bool graphable = n >= 2;
+  for (int32_t i = 0; i < n && graphable; ++i) {
+    graphable = solvers[i]->stream != nullptr && solvers[i]->p.device == solvers[0]->p.device;
+    for (int32_t j = 0; j < i && graphable; ++j) graphable = solvers[j] != solvers[i];
+  }
+  int64_t left = n_steps;
+  if (graphable && left > 0) {
+    cudaStream_t s0 = solvers[0]->stream;
+    // the graph runs in solver 0's stream: it starts after the work already queued in the other streams ...
+    for (int32_t i = 1; i < n; ++i) {
+      if (solvers[i]->stream == s0) continue;
+      HR_CUDA(cudaEventRecord(solvers[i]->relax_ev[0], solvers[i]->stream));
+      HR_CUDA(cudaStreamWaitEvent(s0, solvers[i]->relax_ev[0], 0));
+    }
+    while (left > 0) {
+      const int k = left >= kManyStepsPerGraph ? kManyStepsPerGraph : (int)left;
+      cudaGraphExec_t exec = many_graph(solvers, n, k);
+      if (!exec) break;  // capture failed: plain round robin below
+      HR_CUDA(cudaGraphLaunch(exec, s0));
+      left -= k;
+    }
+    // ... and whatever is queued in them next waits for it
+    HR_CUDA(cudaEventRecord(solvers[0]->relax_ev[1], s0));
+    for (int32_t i = 1; i < n; ++i)
+      if (solvers[i]->stream != s0) HR_CUDA(cudaStreamWaitEvent(solvers[i]->stream, solvers[0]->relax_ev[1], 0));
+  }
+  for (int64_t it = 0; it < left; ++it)
     for (int32_t i = 0; i < n; ++i) HR_TRY(hr_step(solvers[i], 1));
   return HR_OK;
 }

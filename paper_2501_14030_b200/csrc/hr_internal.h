@@ -141,6 +141,8 @@ struct hr_solver {
   int num_sms;
   int march_grid_lean[7] = {0, 0, 0, 0, 0, 0, 0};  // variant 0: the ACC-free stages, by stage % 10
   int march_grid[7];  // persistent grid size per stage kernel (0 = eval, 1..4, 5 = residual, 6 = 1 + residual)
+  int march_slots[7] = {0, 0, 0, 0, 0, 0, 0};       // resident CTAs per SM x SMs, before the clamp to the work
+  int march_slots_lean[7] = {0, 0, 0, 0, 0, 0, 0};
   // TMA descriptors of the ten stored grid functions (Y, A, B, ACC (u, v), psi, S): the TW x BY
   // box of each, and the halo-tile box of the three stencil sources Y_u, A_u, B_u
   CUtensorMap tm_box[10];
@@ -195,6 +197,10 @@ MarchPlan hrk_make_plan(const int32_t n[3], int ng, int coord, int dtype);
 // shared-memory opt-in and persistent grid sizes of the marching kernels; before graph capture
 cudaError_t hrk_prepare(hr_solver* s);
 int hrk_max_partials(const int32_t n[3], int ng, int dtype);
+// Re-chunk the marching plan for a solver that shares the device with `share` - 1 others running at the same
+// time (hr_step_many): chunk lengths and persistent grids as if 1/share of the CTA slots were its own.  share = 1
+// restores the stand-alone plan.  Kernels already captured in a graph keep the plan they were captured with.
+void hrk_replan(hr_solver* s, int share);
 int hrk_launches_per_substep(const hr_solver* s);
 
 // ---- hr_measure.cu ----

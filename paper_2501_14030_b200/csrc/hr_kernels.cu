@@ -10,6 +10,8 @@
 // Product code: nothing here includes, links or calls oracle/.
 #include <cuda_runtime.h>
 
+#include <algorithm>
+
 #include <cstdlib>
 #include <type_traits>
 
@@ -713,13 +715,11 @@ cudaError_t prepare_march(hr_solver* s) {
     if ((e = prepare_march_stage<T, NG, LeanCode<T>::S4>(s, &s->march_grid_lean[4])) != cudaSuccess) return e;
     if ((e = prepare_march_stage<T, NG, 16>(s, &s->march_grid_lean[6])) != cudaSuccess) return e;
   }
-  // one chunking for all stages, balanced for the RK stage kernels (stages 2, 3 dominate)
-  choose_chunks(s->plan, s->g.n2, NG, s->march_grid[2], sizeof(T) == 8);
-  const long long items = (long long)s->plan.ntx * s->plan.nty * s->plan.nzc;
   for (int st = 0; st < 7; ++st) {
-    if (s->march_grid[st] > items) s->march_grid[st] = (int)items;
-    if (s->march_grid_lean[st] > items) s->march_grid_lean[st] = (int)items;
+    s->march_slots[st] = s->march_grid[st];
+    s->march_slots_lean[st] = s->march_grid_lean[st];
   }
+  hrk_replan(s, 1);
   return cudaSuccess;
 }
 
@@ -905,6 +905,19 @@ MarchPlan hrk_make_plan(const int32_t n[3], int ng, int coord, int dtype) {
   m.gt = m.ntx * m.nty;
   (void)ng;
   return m;
+}
+
+void hrk_replan(hr_solver* s, int share) {
+  if (s->p.variant == 1 || s->p.variant == 2) return;
+  if (share < 1) share = 1;
+  // one chunking for all stages, balanced for the RK stage kernels (stages 2, 3 dominate)
+  const int slots = s->march_slots[2] / share > 0 ? s->march_slots[2] / share : 1;
+  choose_chunks(s->plan, s->g.n2, s->g.ng, slots, s->p.dtype == HR_F64);
+  const long long items = (long long)s->plan.ntx * s->plan.nty * s->plan.nzc;
+  for (int st = 0; st < 7; ++st) {
+    s->march_grid[st] = (int)std::min<long long>(s->march_slots[st], items);
+    s->march_grid_lean[st] = (int)std::min<long long>(s->march_slots_lean[st], items);
+  }
 }
 
 cudaError_t hrk_prepare(hr_solver* s) {
