@@ -50,7 +50,11 @@ typedef enum {
   HR_ERR_NUMERIC = 5      /* a puncture coincides with a grid point (non-finite source)       */
 } hr_status;
 
-typedef enum { HR_SINHSPHERICAL = 0, HR_SINHSYMTP = 1 } hr_coord; /* reading C4            */
+/* Reference metrics ("Cartesian-like, spherical-like, cylindrical-like, and bispherical-like"):
+ * SinhSpherical and SinhSymTP (reading C4: x0 in [0,1], x1 = theta in [0,pi], x2 = phi) and SinhCylindrical
+ * (reading C24: x0 in [0,1] -> R = rho(x0), x1 in [-1,1] -> Z = rho(x1), same amp and sinhw, x2 = phi; outer
+ * points beyond the outer cylinder AND beyond both end faces; default and running-sum arrangements only). */
+typedef enum { HR_SINHSPHERICAL = 0, HR_SINHSYMTP = 1, HR_SINHCYLINDRICAL = 2 } hr_coord;
 typedef enum { HR_F64 = 0, HR_F32 = 1 } hr_dtype;                 /* reading C19           */
 
 /* One Brandt-Bruegmann puncture: bare mass, Cartesian position, Bowen-York

@@ -51,12 +51,14 @@ hr_status validate(const hr_params* p) {
   if (!p) return fail(HR_ERR_INVALID_ARG, "params is NULL");
   if (p->fd_order % 2 != 0 || p->fd_order < 2 || p->fd_order > 2 * HR_MAX_NG)
     return fail(HR_ERR_UNSUPPORTED, "fd_order %d not in {2,4,...,%d}", p->fd_order, 2 * HR_MAX_NG);
-  if (p->coord != HR_SINHSPHERICAL && p->coord != HR_SINHSYMTP)
+  if (p->coord != HR_SINHSPHERICAL && p->coord != HR_SINHSYMTP && p->coord != HR_SINHCYLINDRICAL)
     return fail(HR_ERR_UNSUPPORTED, "coord %d unknown", p->coord);
   if (p->dtype != HR_F64 && p->dtype != HR_F32)
     return fail(HR_ERR_UNSUPPORTED, "dtype %d unknown", p->dtype);
   if (p->variant < 0 || p->variant > 3)
     return fail(HR_ERR_UNSUPPORTED, "variant %d unknown", p->variant);
+  if (p->coord == HR_SINHCYLINDRICAL && (p->variant == 1 || p->variant == 2))
+    return fail(HR_ERR_UNSUPPORTED, "SinhCylindrical runs in the marching arrangements (variant 0 or 3) only");
   const int ng = p->fd_order / 2;
   for (int a = 0; a < 3; ++a)
     if (p->n[a] < ng)
@@ -88,6 +90,7 @@ struct Layout {
   size_t off_field[10];
   size_t off_plane[6];
   size_t off_rad[3];
+  size_t off_opos;
   size_t off_wvol, off_inner_dst, off_inner_src, off_partials, off_result, off_counters;
   size_t off_rho, off_rhoz, off_sinth, off_costh, off_sinph, off_cosph, off_punct;
   size_t total;
@@ -101,7 +104,11 @@ Layout make_layout(const hr_params* p) {
   L.ng = p->fd_order / 2;
   for (int a = 0; a < 3; ++a) L.T[a] = p->n[a] + 2 * L.ng;
   L.ntot = (int64_t)L.T[0] * L.T[1] * L.T[2];
-  L.n_inner = L.ntot - (int64_t)p->n[0] * p->n[1] * p->n[2] - (int64_t)L.ng * p->n[1] * p->n[2];
+  // outer points (C13): NG layers beyond x0 at interior angles; C24: beyond the cylinder (all x1) and both ends
+  const int64_t n_outer = p->coord == HR_SINHCYLINDRICAL
+                              ? ((int64_t)L.ng * L.T[1] + 2 * (int64_t)L.ng * p->n[0]) * p->n[2]
+                              : (int64_t)L.ng * p->n[1] * p->n[2];
+  L.n_inner = L.ntot - (int64_t)p->n[0] * p->n[1] * p->n[2] - n_outer;
   const size_t w = p->dtype == HR_F64 ? 8 : 4;
   hrk_row_geometry(L.T[0], L.ng, w, &L.P0, &L.off0);
   L.npad = (int64_t)L.P0 * L.T[1] * L.T[2];
@@ -114,7 +121,10 @@ Layout make_layout(const hr_params* p) {
   for (int f = 0; f < 10; ++f) L.off_field[f] = take((size_t)L.npad * w);
   const size_t np = (size_t)L.T[0] * L.T[1];
   for (int f = 0; f < 6; ++f) L.off_plane[f] = take(np * w);
-  for (int f = 0; f < 3; ++f) L.off_rad[f] = take((size_t)L.ng * L.T[1] * w);
+  // outer positions in the (i0,i1) plane: NG columns beyond x0 (all rows) + 2 NG rows beyond x1 (C24)
+  const size_t n_o2_max = (size_t)L.ng * L.T[1] + 2 * (size_t)L.ng * L.T[0];
+  for (int f = 0; f < 3; ++f) L.off_rad[f] = take(n_o2_max * w);
+  L.off_opos = take(n_o2_max * 4);
   L.off_wvol = take(np * 8);
   L.off_inner_dst = take((size_t)L.n_inner * 4 + 4);
   L.off_inner_src = take((size_t)L.n_inner * 4 + 4);
@@ -155,10 +165,25 @@ Radial radial_map(const hr_params& p, double x0) {
   return r;
 }
 
-MetricPoint metric_point(const hr_params& p, const Radial& R, double sth, double cth) {
+// (SinhCylindrical, reading C24: Z = the same sinh map evaluated at x1.)
+MetricPoint metric_point(const hr_params& p, const Radial& R, double sth, double cth, const Radial& Z) {
   MetricPoint m;
   const double A = R.f, A1 = R.d1, A2 = R.d2;
-  if (p.coord == HR_SINHSPHERICAL) {
+  if (p.coord == HR_SINHCYLINDRICAL) {
+    // flat metric in cylindrical coordinates (R(x0), Z(x1), phi): h = (R', Z', R)
+    m.h0 = A1;
+    m.h1 = Z.d1;
+    m.h2 = A;
+    m.g00 = 1.0 / (A1 * A1);
+    m.g11 = 1.0 / (Z.d1 * Z.d1);
+    m.g22 = 1.0 / (A * A);
+    m.g0 = (1.0 / A - A2 / (A1 * A1)) / A1;
+    m.g1 = -Z.d2 / (Z.d1 * Z.d1 * Z.d1);
+    const double r = std::sqrt(A * A + Z.f * Z.f);  // distance from the grid centre
+    m.rad0 = A / (r * A1);
+    m.rad1 = Z.f / (r * Z.d1);
+    m.invr = 1.0 / r;
+  } else if (p.coord == HR_SINHSPHERICAL) {
     // flat metric in spherical coordinates with r = rho(x0)
     m.h0 = A1;
     m.h1 = A;
@@ -206,7 +231,9 @@ inline void inner_source(const hr_params& p, int ng, const int T[3], int i0, int
     ++flips;
     if (p.coord == HR_SINHSPHERICAL) j1 = T[1] - 1 - j1;  // r -> -r also sends theta -> pi - theta
   }
-  if (j1 < ng) {  // theta -> -theta
+  if (p.coord == HR_SINHCYLINDRICAL) {
+    // C24: x1 is the axial coordinate, points beyond its ends are outer points, nothing reflects
+  } else if (j1 < ng) {  // theta -> -theta
     j1 = 2 * ng - 1 - j1;
     ++flips;
   } else if (j1 >= N1 + ng) {  // theta -> 2 pi - theta
@@ -249,6 +276,11 @@ struct HostSetup {
   std::vector<double> rho, rhoz, sth, cth, sph, cph;           // 1-D coordinate tables
   std::vector<double> l00, l11, l22, l0, l1, c2, wv;           // (i0,i1) planes
   std::vector<double> r0, r1, ri;                              // compact outer planes (ng x T1)
+  // the outer positions of the (i0,i1) plane in ascending order, what the kernels walk (C13): position
+  // i0 + T0 i1 in the low 28 bits, stencil bits above (1: beyond x0, backward d_0; 2: beyond the high end
+  // of x1, backward d_1; 4: beyond the low end of x1, forward d_1; centred otherwise) and their factors
+  std::vector<int32_t> opos;
+  std::vector<double> o_r0, o_r1, o_ri;
   std::vector<int32_t> inner_dst, inner_src, outer_idx;
 };
 
@@ -258,10 +290,12 @@ hr_status host_setup(const hr_params* p, HostSetup& H) {
   const int T0 = H.T[0], T1 = H.T[1], T2 = H.T[2];
   const int n0 = p->n[0], n1 = p->n[1], n2 = p->n[2];
   // ---- Alg. 1 l.2: cell-centred coordinate tables (C8) ----
+  const bool cyl = p->coord == HR_SINHCYLINDRICAL;
   H.dx[0] = 1.0 / n0;
-  H.dx[1] = kPi / n1;
+  H.dx[1] = (cyl ? 2.0 : kPi) / n1;
   H.dx[2] = 2.0 * kPi / n2;
-  std::vector<Radial> R(T0);
+  if ((int64_t)T0 * T1 >= (1 << 28)) return fail(HR_ERR_INVALID_ARG, "T0 * T1 exceeds 2^28");
+  std::vector<Radial> R(T0), Zt(T1);
   H.rho.resize(T0); H.rhoz.resize(T0); H.sth.resize(T1); H.cth.resize(T1); H.sph.resize(T2);
   H.cph.resize(T2);
   for (int i = 0; i < T0; ++i) {
@@ -269,11 +303,18 @@ hr_status host_setup(const hr_params* p, HostSetup& H) {
     H.rho[i] = R[i].f;
     H.rhoz[i] =
         p->coord == HR_SINHSYMTP ? std::sqrt(R[i].f * R[i].f + p->bscale * p->bscale) : R[i].f;
+    if (cyl) H.rhoz[i] = 1.0;  // the source kernel forms z = rhoz[i0] * costh[i1]: here z = Z(x1)
   }
   for (int i = 0; i < T1; ++i) {
     const double th = (i - ng + 0.5) * H.dx[1];
     H.sth[i] = std::sin(th);
     H.cth[i] = std::cos(th);
+    Zt[i] = Radial{0.0, 0.0, 0.0};
+    if (cyl) {  // x1 in [-1,1]; (x, y, z) = (R cos phi, R sin phi, Z)
+      Zt[i] = radial_map(*p, -1.0 + (i - ng + 0.5) * H.dx[1]);
+      H.sth[i] = 1.0;
+      H.cth[i] = Zt[i].f;
+    }
   }
   for (int i = 0; i < T2; ++i) {
     const double ph = -kPi + (i - ng + 0.5) * H.dx[2];
@@ -290,7 +331,7 @@ hr_status host_setup(const hr_params* p, HostSetup& H) {
   for (int i1 = 0; i1 < T1; ++i1)
     for (int i0 = 0; i0 < T0; ++i0) {
       const size_t q = (size_t)i0 + (size_t)T0 * i1;
-      const MetricPoint m = metric_point(*p, R[i0], H.sth[i1], H.cth[i1]);
+      const MetricPoint m = metric_point(*p, R[i0], H.sth[i1], H.cth[i1], Zt[i1]);
       mp[q] = m;
       const double d = std::fmin(std::fabs(m.h0) * H.dx[0],
                                  std::fmin(std::fabs(m.h1) * H.dx[1], std::fabs(m.h2) * H.dx[2]));
@@ -321,22 +362,33 @@ hr_status host_setup(const hr_params* p, HostSetup& H) {
         H.r1[qo] = c * m.rad1 / (2.0 * H.dx[1]);
         H.ri[qo] = c * m.invr;
       }
+      const bool in1 = i1 >= ng && i1 < n1 + ng;
+      const bool outer = i0 >= ng && (cyl ? (i0 >= n0 + ng || !in1) : (i0 >= n0 + ng && in1));
+      if (outer) {
+        const int bits = (i0 >= n0 + ng ? 1 : 0) | (i1 >= n1 + ng ? 2 : 0) | (i1 < ng ? 4 : 0);
+        H.opos.push_back((int32_t)q | (bits << 28));
+        H.o_r0.push_back(c * m.rad0 / (2.0 * H.dx[0]));
+        H.o_r1.push_back(c * m.rad1 / (2.0 * H.dx[1]));
+        H.o_ri.push_back(c * m.invr);
+      }
     }
 
   // ---- Alg. 1 l.4: boundary containers (C13, C14), ascending destination index ----
   const int64_t ntot = (int64_t)T0 * T1 * T2;
-  const int64_t n_outer = (int64_t)ng * n1 * n2;
+  const int64_t n_outer = (int64_t)H.opos.size() * n2;
   const int64_t n_inner = ntot - (int64_t)n0 * n1 * n2 - n_outer;
   H.inner_dst.reserve((size_t)n_inner);
   H.inner_src.reserve((size_t)n_inner);
   H.outer_idx.reserve((size_t)n_outer);
   for (int i2 = 0; i2 < T2; ++i2)
     for (int i1 = 0; i1 < T1; ++i1) {
-      const bool in12 = i1 >= ng && i1 < n1 + ng && i2 >= ng && i2 < n2 + ng;
+      const bool in1 = i1 >= ng && i1 < n1 + ng, in2 = i2 >= ng && i2 < n2 + ng;
       for (int i0 = 0; i0 < T0; ++i0) {
-        if (in12 && i0 >= ng) {
-          if (i0 >= n0 + ng) H.outer_idx.push_back(i0 + T0 * (i1 + T1 * i2));
-          continue;  // interior or outer
+        const bool in0 = i0 >= ng && i0 < n0 + ng;
+        if (in0 && in1 && in2) continue;  // interior
+        if (in2 && i0 >= ng && (cyl ? (i0 >= n0 + ng || !in1) : (i0 >= n0 + ng && in1))) {
+          H.outer_idx.push_back(i0 + T0 * (i1 + T1 * i2));
+          continue;  // outer
         }
         int j0, j1, j2;
         inner_source(*p, ng, H.T, i0, i1, i2, j0, j1, j2);
@@ -413,7 +465,7 @@ hr_status hr_create(const hr_params* p, void* workspace_dev, size_t workspace_by
   g.ntot = L.ntot;
   g.n_inner = L.n_inner;
   g.n_outer_cols = ng;
-  s->n_outer = (int64_t)ng * g.n1 * g.n2;
+  s->n_outer = 0;  // set from the host tables below
   s->max_partials = L.nblocks;
   s->plan = hrk_make_plan(p->n, ng, p->coord, p->dtype);
   HR_CUDA(cudaDeviceGetAttribute(&s->num_sms, cudaDevAttrMultiProcessorCount, p->device));
@@ -428,6 +480,7 @@ hr_status hr_create(const hr_params* p, void* workspace_dev, size_t workspace_by
   a.L00 = base + L.off_plane[0]; a.L11 = base + L.off_plane[1]; a.L22 = base + L.off_plane[2];
   a.L0 = base + L.off_plane[3];  a.L1 = base + L.off_plane[4];  a.C2 = base + L.off_plane[5];
   a.RAD0 = base + L.off_rad[0]; a.RAD1 = base + L.off_rad[1]; a.RADI = base + L.off_rad[2];
+  a.OPOS = reinterpret_cast<int32_t*>(base + L.off_opos);
   a.Wvol = reinterpret_cast<double*>(base + L.off_wvol);
   a.inner_dst = reinterpret_cast<int32_t*>(base + L.off_inner_dst);
   a.inner_src = reinterpret_cast<int32_t*>(base + L.off_inner_src);
@@ -469,9 +522,12 @@ hr_status hr_create(const hr_params* p, void* workspace_dev, size_t workspace_by
   HR_TRY(upload_plane(s, a.L0, H.l0));
   HR_TRY(upload_plane(s, a.L1, H.l1));
   HR_TRY(upload_plane(s, a.C2, H.c2));
-  HR_TRY(upload_plane(s, a.RAD0, H.r0));
-  HR_TRY(upload_plane(s, a.RAD1, H.r1));
-  HR_TRY(upload_plane(s, a.RADI, H.ri));
+  HR_TRY(upload_plane(s, a.RAD0, H.o_r0));
+  HR_TRY(upload_plane(s, a.RAD1, H.o_r1));
+  HR_TRY(upload_plane(s, a.RADI, H.o_ri));
+  HR_TRY(upload(a.OPOS, H.opos.data(), H.opos.size() * 4, s->stream));
+  s->n_outer = (int64_t)s->outer_idx.size();
+  s->g.n_o2 = (int32_t)H.opos.size();
   HR_TRY(upload(a.Wvol, H.wv.data(), np * 8, s->stream));
   {
     // device copies of the inner lists in stored (padded) indices; the host copies stay public

@@ -30,6 +30,7 @@ struct HrGrid {
   int64_t ntot;
   int64_t n_inner;
   int32_t n_outer_cols;  // = ng: outer layers i0 in [n0+ng, T0)
+  int32_t n_o2;          // outer positions of the (i0,i1) plane (HrArrays::OPOS); outer points = n_o2 * n2
 };
 
 // Pointers into the caller's workspace.  `void*` scalars are double or float per dtype.
@@ -52,6 +53,9 @@ struct HrArrays {
   void* RAD0;  // c * rad0 / (2 dx0)
   void* RAD1;  // c * rad1 / (2 dx1)
   void* RADI;  // c / r
+  // the outer positions themselves: i0 + T0 i1 in the low 28 bits, stencil bits above (hr_api.cu: HostSetup::opos);
+  // RAD0 / RAD1 / RADI are indexed like this list
+  int32_t* OPOS;
   double* Wvol;  // |h0 h1 h2| plane, always fp64 (C16)
   int32_t* inner_dst;
   int32_t* inner_src;
@@ -132,6 +136,7 @@ struct MarchPlan {
   int gt;        // tiles per group (whole tile rows); items are chunk-major within a group
   int* counters; // device: {next item, CTAs done} per stage kernel, zero between launches
   int sph;       // 1 = SinhSpherical inner map (theta -> pi - theta under rho -> -rho)
+  int cyl;       // 1 = SinhCylindrical (C24): x1 is axial, no theta reflections, outer points beyond its ends
   int* flag;     // device: set non-zero by a kernel that meets psi_BL + u <= 0 or NaN at an interior point
 };
 

@@ -63,6 +63,7 @@ struct StepArgs {
   const T* S;
   const T *L00, *L11, *L22, *L0, *L1, *C2;
   const T *RAD0, *RAD1, *RADI;
+  const int32_t* OPOS;  // outer positions of the (i0,i1) plane with their stencil bits (C13)
   T eta;
   T dt;
 };
@@ -155,12 +156,19 @@ __device__ __forceinline__ T laplacian_direct(const T* __restrict__ u, int64_t c
 
 // Radiation condition (C13) at an outer point c = (i0,i1,i2), j = i0 - (n0+ng):
 //   k_f = -c [ rad0 (3 f_i - 4 f_{i-1} + f_{i-2})/(2 dx0) + rad1 (f_{i1+1} - f_{i1-1})/(2 dx1) + f/r ]
+// Each derivative is second order: one-sided, pointing into the grid, along an axis in which the point lies
+// beyond the interior (bits: 1 beyond x0 -> backward d_0; 2 beyond the high end of x1 -> backward d_1; 4 beyond
+// its low end -> forward d_1), centred otherwise.  Spherical-like systems: bits = 1 at every outer point.
 template <typename T>
 __device__ __forceinline__ T radiation_k(const T* __restrict__ f, int64_t c, int64_t s1, T r0,
-                                         T r1, T ri) {
+                                         T r1, T ri, int bits = 1) {
   const T fc = f[c];
-  const T d0 = T(3) * fc - T(4) * f[c - 1] + f[c - 2];
-  const T d1 = f[c + s1] - f[c - s1];
+  T d0, d1;
+  if (bits & 1) d0 = T(3) * fc - T(4) * f[c - 1] + f[c - 2];
+  else d0 = f[c + 1] - f[c - 1];
+  if (bits & 2) d1 = T(3) * fc - T(4) * f[c - s1] + f[c - 2 * s1];
+  else if (bits & 4) d1 = T(4) * f[c + s1] - T(3) * fc - f[c + 2 * s1];
+  else d1 = f[c + s1] - f[c - s1];
   return -(r0 * d0 + r1 * d1 + ri * fc);
 }
 
@@ -186,7 +194,7 @@ __global__ void __launch_bounds__(DBX* DBY)
     ku = vc - a.eta * uc;
     kv = a.C2[q] * (lap + a.S[c] * pow_m7(a.psi[c] + uc));
   } else {
-    const int qo = (i0 - (g.n0 + NG)) + NG * i1;
+    const int qo = (i0 - (g.n0 + NG)) + NG * (i1 - NG);  // position in the outer list (HrArrays::OPOS order)
     const T r0 = a.RAD0[qo], r1 = a.RAD1[qo], ri = a.RADI[qo];
     ku = radiation_k(a.in_u, c, g.s1, r0, r1, ri);
     kv = radiation_k(a.in_v, c, g.s1, r0, r1, ri);
@@ -226,7 +234,7 @@ __global__ void __launch_bounds__(256)
   const int r = m / NG;
   const int i1 = NG + r % g.n1, i2 = NG + r / g.n1;
   const int64_t c = g.off0 + (g.n0 + NG + j) + g.s1 * i1 + g.s2 * i2;
-  const int qo = j + NG * i1;
+  const int qo = j + NG * (i1 - NG);  // position in the outer list (HrArrays::OPOS order)
   const T r0 = a.RAD0[qo], r1 = a.RAD1[qo], ri = a.RADI[qo];
   a.out_u[c] = radiation_k(a.in_u, c, g.s1, r0, r1, ri);
   a.out_v[c] = radiation_k(a.in_v, c, g.s1, r0, r1, ri);
@@ -481,6 +489,7 @@ StepArgs<T> make_args(const hr_solver* s, int stage, void* ku, void* kv) {
   r.psi = P(a.psi); r.S = P(a.S);
   r.L00 = P(a.L00); r.L11 = P(a.L11); r.L22 = P(a.L22); r.L0 = P(a.L0); r.L1 = P(a.L1);
   r.C2 = P(a.C2); r.RAD0 = P(a.RAD0); r.RAD1 = P(a.RAD1); r.RADI = P(a.RADI);
+  r.OPOS = a.OPOS;
   r.eta = (T)s->p.eta;
   r.dt = (T)s->dt;
   return r;
@@ -900,6 +909,7 @@ MarchPlan hrk_make_plan(const int32_t n[3], int ng, int coord, int dtype) {
   m.ntx = (n[0] + tw - 1) / tw;
   m.nty = (n[1] + by - 1) / by;
   m.sph = coord == HR_SINHSPHERICAL ? 1 : 0;
+  m.cyl = coord == HR_SINHCYLINDRICAL ? 1 : 0;
   m.zc = n[2];
   m.nzc = 1;
   m.gt = m.ntx * m.nty;

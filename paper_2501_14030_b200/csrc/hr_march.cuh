@@ -464,18 +464,18 @@ __global__ void __launch_bounds__((TW / VX) * BY,
   // first TMA loads of its first item, so that its load latency hides behind theirs (on L2-resident
   // grids a CTA lives for one short item: anything serial at its end is on the critical path).
   [[maybe_unused]] auto outer_tail = [&]() {
-    const int n_outer = NG * g.n1 * g.n2;
+    const int n_outer = g.n_o2 * g.n2;
     for (int m = blockIdx.x * NT + tid; m < n_outer; m += gridDim.x * NT) {
-      const int j = m % NG;
-      const int r = m / NG;
-      const int i1 = NG + r % g.n1, i2 = NG + r / g.n1;
-      const int i0 = g.n0 + NG + j;
+      const int qo = m % g.n_o2;
+      const int i2 = NG + m / g.n_o2;
+      const int po = a.OPOS[qo];
+      const int bits = po >> 28, q = po & 0x0fffffff;
+      const int i1 = q / g.T0, i0 = q - i1 * g.T0;
       const int c = g.off0 + i0 + g.P0 * i1 + s2 * i2;
-      const int qo = j + NG * i1;
       const T r0 = a.RAD0[qo], r1 = a.RAD1[qo], ri = a.RADI[qo];
       const T uc = a.in_u[c], vc = a.in_v[c];
-      const T ku = radiation_k(a.in_u, c, g.P0, r0, r1, ri);
-      const T kv = radiation_k(a.in_v, c, g.P0, r0, r1, ri);
+      const T ku = radiation_k(a.in_u, c, g.P0, r0, r1, ri, bits);
+      const T kv = radiation_k(a.in_v, c, g.P0, r0, r1, ri, bits);
       T wu, wv;
       if constexpr (LEAN) {
         T yu = T(0), yv = T(0);
@@ -499,10 +499,12 @@ __global__ void __launch_bounds__((TW / VX) * BY,
       } else {
         rk_combine<T, RK>(a, c, ku, kv, uc, vc, wu, wv);
       }
-      const int cB = i1 < 2 * NG ? 2 * NG - 1 - i1 : -1;
-      const int cC = i1 >= g.n1 ? 2 * (g.n1 + NG) - 1 - i1 : -1;
-      if (cB >= 0 || cC >= 0 || i2 < 2 * NG || i2 >= g.n2)
-        scatter_images<T>(ig, a.out_u, a.out_v, wu, wv, i0, i1, i2, -1, cB, cC);
+      // theta reflections (spherical-like systems); rho -> -rho images of the end-face points near the axis (C24)
+      const int cB = (!plan.cyl && i1 < 2 * NG) ? 2 * NG - 1 - i1 : -1;
+      const int cC = (!plan.cyl && i1 >= g.n1) ? 2 * (g.n1 + NG) - 1 - i1 : -1;
+      const int rr = i0 < 2 * NG ? 2 * NG - 1 - i0 : -1;
+      if (cB >= 0 || cC >= 0 || rr >= 0 || i2 < 2 * NG || i2 >= g.n2)
+        scatter_images<T>(ig, a.out_u, a.out_v, wu, wv, i0, i1, i2, rr, cB, cC);
     }
   };
   [[maybe_unused]] bool tail_done = false;
@@ -588,7 +590,7 @@ __global__ void __launch_bounds__((TW / VX) * BY,
         }
       }
     }
-    if (ADVANCE && nact > 0) {
+    if (ADVANCE && nact > 0 && !plan.cyl) {
       cB = i1 < 2 * NG ? 2 * NG - 1 - i1 : -1;
       cC = i1 >= g.n1 ? 2 * (g.n1 + NG) - 1 - i1 : -1;
       inplane_images |= (cB >= 0) || (cC >= 0);

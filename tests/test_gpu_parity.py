@@ -50,6 +50,10 @@ SMALL = [
     ("tp_o2", W.sweep_point(4, (20, 10, 8), "SinhSymTP", 2)),
     ("sph_o12", W.sweep_point(5, (24, 12, 12), "SinhSpherical", 12)),
     ("minimal_o10", W.sweep_point(6, (5, 5, 6), "SinhSymTP", 10)),
+    # cylindrical-like reference metric (reading C24): outer points on three faces
+    ("cyl_o4", W.sweep_point(8, (40, 24, 16), "SinhCylindrical", 4)),
+    ("cyl_o8_ragged", W.sweep_point(9, (33, 19, 10), "SinhCylindrical", 8)),
+    ("cyl_o10_ragged", W.sweep_point(10, (35, 37, 12), "SinhCylindrical", 10)),
 ]
 
 
@@ -151,7 +155,10 @@ def test_rhs_pointwise_conditioned_error(hr, name, params):
 
 STEP_CASES = [("config0", W.config(0), 200), ("config1_half", dict(W.config(1, scale=0.5), eta=30.0), 400),
               ("config3_eighth", dict(W.config(3, scale=0.125), eta=60.0), 200),
-              ("sph_o6_ragged", dict(W.sweep_point(0, (70, 18, 10), "SinhSpherical", 6), eta=2.0), 100)]
+              ("sph_o6_ragged", dict(W.sweep_point(0, (70, 18, 10), "SinhSpherical", 6), eta=2.0), 100),
+              # (eta dt must stay well below RK4's real-axis limit 2.78, C10: dt = 3.2 and 1.7 on these coarse grids)
+              ("cyl_o8_ragged", dict(W.sweep_point(9, (33, 38, 10), "SinhCylindrical", 8), eta=0.2), 100),
+              ("cyl_o4", dict(W.sweep_point(8, (40, 48, 16), "SinhCylindrical", 4), eta=0.2), 200)]
 
 
 @pytest.mark.parametrize("name,params,steps", STEP_CASES, ids=[c[0] for c in STEP_CASES])
