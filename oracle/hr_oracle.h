@@ -35,8 +35,8 @@ extern "C" {
 #endif
 
 /* "Cartesian-like, spherical-like, cylindrical-like, and bispherical-like" reference metrics.
- * 0, 1: readings C4; 2: reading C24. */
-enum { ORC_SINHSPHERICAL = 0, ORC_SINHSYMTP = 1, ORC_SINHCYLINDRICAL = 2 };
+ * 0, 1: readings C4; 2: reading C24; 3: reading C25. */
+enum { ORC_SINHSPHERICAL = 0, ORC_SINHSYMTP = 1, ORC_SINHCYLINDRICAL = 2, ORC_SINHCARTESIAN = 3 };
 
 /* One puncture = 10 doubles: m, pos[3], P[3], S[3] (Cartesian). */
 typedef struct {
@@ -69,6 +69,11 @@ void orc_get_source(const orc_grid* g, double* psi, double* S);   /* ntot each, 
  * wave speed c (C9), volume weight |h0 h1 h2| (C16), local spacing ds (C9). */
 void orc_get_planes(const orc_grid* g, double* g00, double* g11, double* g22, double* g0,
                     double* g1, double* c, double* w, double* ds);
+/* C25 only (SinhCartesian): what depends on x2, T2 doubles each: the u_22 and u_2 factors 1/h2^2 and
+ * -X2''/X2'^3, the spacing h2 dx2 and h2.  There lap u = g00 u_00 + g11 u_11 + z22 u_22 + g0 u_0 + g1 u_1
+ * + z2 u_2, ds = min(ds plane, zds), |h0 h1 h2| = w plane * zh, and the c plane holds c_min ds_plane/ds_min.
+ * For the other systems: 1, 0, +inf, 1. */
+void orc_get_axis2(const orc_grid* g, double* z22, double* z2, double* zds, double* zh);
 
 /* ---- stand-alone pieces exposed for the pins ---- */
 /* C11: centred weights; c1[0..n] (c1[0]=0), d2[0..n], n = order/2, unit spacing. */

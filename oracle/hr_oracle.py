@@ -13,6 +13,7 @@ from . import build as _build
 SINHSPHERICAL = 0
 SINHSYMTP = 1
 SINHCYLINDRICAL = 2
+SINHCARTESIAN = 3
 
 _i32p = C.POINTER(C.c_int32)
 _f64p = C.POINTER(C.c_double)
@@ -123,7 +124,7 @@ class Oracle:
         self._punct = _punct_array(params["punctures"])
         p = _Params()
         p.n[:] = [int(x) for x in params["n"]]
-        p.coord = {"SinhSpherical": 0, "SinhSymTP": 1, "SinhCylindrical": 2}[params["coord"]]
+        p.coord = {"SinhSpherical": 0, "SinhSymTP": 1, "SinhCylindrical": 2, "SinhCartesian": 3}[params["coord"]]
         p.fd_order = int(params["fd_order"])
         p.n_punctures = int(self._punct.shape[0])
         p.amp = float(params["amp"])
@@ -182,6 +183,13 @@ class Oracle:
         names = ["g00", "g11", "g22", "g0", "g1", "c", "w", "ds"]
         arrs = [np.zeros((self.T[1], self.T[0])) for _ in names]
         lib().orc_get_planes(self._h, *[_ptr(a) for a in arrs])
+        return dict(zip(names, arrs))
+
+    def axis2(self):
+        """C25: the x2-dependent factors z22, z2, zds, zh (T2 each); 1, 0, inf, 1 for the other systems."""
+        names = ["z22", "z2", "zds", "zh"]
+        arrs = [np.zeros(self.T[2]) for _ in names]
+        lib().orc_get_axis2(self._h, *[_ptr(a) for a in arrs])
         return dict(zip(names, arrs))
 
     def interior_mask(self):

@@ -83,6 +83,15 @@ void orc_map_to_cart(int32_t coord, double amp, double sinhw, double bscale, dou
     xyz[2] = z;
     return;
   }
+  if (coord == ORC_SINHCARTESIAN) { /* C25: x^a in [-1,1], X_a = rho(x^a), the same sinh map on every axis */
+    double t, tp, tpp;
+    xyz[0] = r;
+    orc_rho(amp, sinhw, x1, &t, &tp, &tpp);
+    xyz[1] = t;
+    orc_rho(amp, sinhw, x2, &t, &tp, &tpp);
+    xyz[2] = t;
+    return;
+  }
   const double st = sin(x1), ct = cos(x1), sp = sin(x2), cp = cos(x2);
   xyz[0] = r * st * cp;
   xyz[1] = r * st * sp;
@@ -100,6 +109,10 @@ void orc_map_from_cart(int32_t coord, double amp, double sinhw, double bscale,
   const double rc2 = x * x + y * y; /* cylindrical radius squared */
   const double rc = sqrt(rc2);
   double rad, th;
+  if (coord == ORC_SINHCARTESIAN) { /* C25: axis by axis */
+    for (int a = 0; a < 3; ++a) x012[a] = sinhw * asinh(xyz[a] * sinh(1.0 / sinhw) / amp);
+    return;
+  }
   if (coord == ORC_SINHCYLINDRICAL) { /* C24: x0 from the cylindrical radius, x1 from z, same sinh map */
     double ph = atan2(y, x);
     if (ph >= ORC_PI) ph -= 2.0 * ORC_PI;
@@ -141,6 +154,21 @@ void orc_metric_at(int32_t coord, double amp, double sinhw, double bscale, doubl
                    double* h, double* gfac) {
   double r, rp, rpp;
   orc_rho(amp, sinhw, x0, &r, &rp, &rpp);
+  if (coord == ORC_SINHCARTESIAN) {
+    /* C25: h_a = X_a'(x^a);  lap u = sum_a [ u_aa / X_a'^2 - X_a''/X_a'^3 u_a ].  The x2 parts (h[2],
+     * gfac[2] and the u_2 factor) are functions of x2 alone: orc_metric_axis2.                    */
+    double t, tp, tpp;
+    orc_rho(amp, sinhw, x1, &t, &tp, &tpp);
+    h[0] = rp;
+    h[1] = tp;
+    h[2] = 1.0;
+    gfac[0] = 1.0 / (rp * rp);
+    gfac[1] = 1.0 / (tp * tp);
+    gfac[2] = 1.0;
+    gfac[3] = -rpp / (rp * rp * rp);
+    gfac[4] = -tpp / (tp * tp * tp);
+    return;
+  }
   if (coord == ORC_SINHCYLINDRICAL) {
     /* C24: h = (R', Z', R);  lap u = u_00/R'^2 + u_11/Z'^2 + u_22/R^2
      *                                + [1/(R R') - R''/R'^3] u_0 - [Z''/Z'^3] u_1               */
@@ -179,6 +207,22 @@ void orc_metric_at(int32_t coord, double amp, double sinhw, double bscale, doubl
     gfac[3] = ((2.0 * r * r + b2) / (r * rp) - AB * rpp / (rp * rp * rp)) / Sg;
     gfac[4] = (ct / st) / Sg;
   }
+}
+
+/* C25: the x2-dependent part of the SinhCartesian metric: h2 = X', u_22 factor 1/X'^2, u_2 factor -X''/X'^3. */
+static void orc_metric_axis2(int32_t coord, double amp, double sinhw, double x2, double* h2, double* g22,
+                             double* g2) {
+  if (coord != ORC_SINHCARTESIAN) {
+    *h2 = 1.0;
+    *g22 = 1.0;
+    *g2 = 0.0;
+    return;
+  }
+  double t, tp, tpp;
+  orc_rho(amp, sinhw, x2, &t, &tp, &tpp);
+  *h2 = tp;
+  *g22 = 1.0 / (tp * tp);
+  *g2 = -tpp / (tp * tp * tp);
 }
 
 /* C13: radial derivative from coordinate derivatives, d_r f = rad0 d_0 f + rad1 d_1 f,
@@ -267,7 +311,8 @@ static int orc_is_interior(const orc_grid* g, int a, int i) {
 
 /* C14: nearest grid index of coordinate x along axis a, and the fractional error. */
 static int orc_nearest_index(const orc_grid* g, int a, double x, double* frac_err) {
-  const double xmin = (a == 2) ? -ORC_PI : ((a == 1 && g->p.coord == ORC_SINHCYLINDRICAL) ? -1.0 : 0.0);
+  double xmin = (a == 2) ? -ORC_PI : ((a == 1 && g->p.coord == ORC_SINHCYLINDRICAL) ? -1.0 : 0.0);
+  if (g->p.coord == ORC_SINHCARTESIAN) xmin = -1.0;
   const double j = (x - xmin) / g->dx[a] - 0.5 + (double)g->ng;
   const double jr = floor(j + 0.5);
   *frac_err = fabs(j - jr);
@@ -282,6 +327,7 @@ static int orc_nearest_index(const orc_grid* g, int a, double x, double* frac_er
  * beyond the domain has no other representative); every other ghost point is an inner point. */
 static int orc_is_outer(const orc_grid* g, int i0, int i1, int i2) {
   const int in1 = orc_is_interior(g, 1, i1), in2 = orc_is_interior(g, 2, i2);
+  if (g->p.coord == ORC_SINHCARTESIAN) return 1; /* C25: no point has a second representative */
   if (!in2 || i0 < g->ng) return 0;
   if (g->p.coord == ORC_SINHCYLINDRICAL) return (i0 >= g->p.n[0] + g->ng) || !in1;
   return (i0 >= g->p.n[0] + g->ng) && in1;
@@ -346,8 +392,7 @@ static int orc_build_bc(orc_grid* g) {
 orc_grid* orc_create(const orc_params* p) {
   if (!p) return NULL;
   if (p->fd_order < 2 || p->fd_order > 2 * ORC_MAX_NG || (p->fd_order % 2)) return NULL;
-  if (p->coord != ORC_SINHSPHERICAL && p->coord != ORC_SINHSYMTP && p->coord != ORC_SINHCYLINDRICAL)
-    return NULL;
+  if (p->coord < ORC_SINHSPHERICAL || p->coord > ORC_SINHCARTESIAN) return NULL;
   const int ng = p->fd_order / 2;
   for (int a = 0; a < 3; ++a)
     if (p->n[a] < ng) return NULL;
@@ -373,16 +418,42 @@ orc_grid* orc_create(const orc_params* p) {
   }
 
   /* C8: cell-centred uniform coordinates, x0 in [0,1], x1 in [0,pi] (C24: [-1,1]), x2 in [-pi,pi]. */
-  const double x1min = (p->coord == ORC_SINHCYLINDRICAL) ? -1.0 : 0.0;
-  g->dx[0] = 1.0 / (double)p->n[0];
-  g->dx[1] = ((p->coord == ORC_SINHCYLINDRICAL) ? 2.0 : ORC_PI) / (double)p->n[1];
-  g->dx[2] = 2.0 * ORC_PI / (double)p->n[2];
+  const int cart = p->coord == ORC_SINHCARTESIAN;
+  const double x1min = (p->coord == ORC_SINHCYLINDRICAL || cart) ? -1.0 : 0.0;
+  const double x0min = cart ? -1.0 : 0.0, x2min = cart ? -1.0 : -ORC_PI;
+  g->dx[0] = (cart ? 2.0 : 1.0) / (double)p->n[0];
+  g->dx[1] = ((p->coord == ORC_SINHCYLINDRICAL || cart) ? 2.0 : ORC_PI) / (double)p->n[1];
+  g->dx[2] = (cart ? 2.0 : 2.0 * ORC_PI) / (double)p->n[2];
   g->x0 = (double*)malloc(sizeof(double) * (size_t)g->T[0]);
   g->x1 = (double*)malloc(sizeof(double) * (size_t)g->T[1]);
   g->x2 = (double*)malloc(sizeof(double) * (size_t)g->T[2]);
-  for (int i = 0; i < g->T[0]; ++i) g->x0[i] = ((double)(i - ng) + 0.5) * g->dx[0];
+  for (int i = 0; i < g->T[0]; ++i) g->x0[i] = x0min + ((double)(i - ng) + 0.5) * g->dx[0];
   for (int i = 0; i < g->T[1]; ++i) g->x1[i] = x1min + ((double)(i - ng) + 0.5) * g->dx[1];
-  for (int i = 0; i < g->T[2]; ++i) g->x2[i] = -ORC_PI + ((double)(i - ng) + 0.5) * g->dx[2];
+  for (int i = 0; i < g->T[2]; ++i) g->x2[i] = x2min + ((double)(i - ng) + 0.5) * g->dx[2];
+  /* C25: x2-dependent factors and, per axis, X_a and 1/h_a (1, 0, +inf, 1 and unused otherwise) */
+  g->z22 = (double*)malloc(sizeof(double) * (size_t)g->T[2]);
+  g->z2 = (double*)malloc(sizeof(double) * (size_t)g->T[2]);
+  g->zds = (double*)malloc(sizeof(double) * (size_t)g->T[2]);
+  g->zh = (double*)malloc(sizeof(double) * (size_t)g->T[2]);
+  for (int i = 0; i < g->T[2]; ++i) {
+    double h2, g22, g2;
+    orc_metric_axis2(p->coord, p->amp, p->sinhw, g->x2[i], &h2, &g22, &g2);
+    g->z22[i] = g22;
+    g->z2[i] = g2;
+    g->zh[i] = h2;
+    g->zds[i] = cart ? fabs(h2) * g->dx[2] : INFINITY;
+  }
+  for (int a = 0; a < 3; ++a) {
+    const double* xa = (a == 0) ? g->x0 : ((a == 1) ? g->x1 : g->x2);
+    g->X[a] = (double*)malloc(sizeof(double) * (size_t)g->T[a]);
+    g->ih[a] = (double*)malloc(sizeof(double) * (size_t)g->T[a]);
+    for (int i = 0; i < g->T[a]; ++i) {
+      double t, tp, tpp;
+      orc_rho(p->amp, p->sinhw, xa[i], &t, &tp, &tpp);
+      g->X[a][i] = t;
+      g->ih[a][i] = 1.0 / tp;
+    }
+  }
 
   orc_fd_weights(p->fd_order, g->c1, g->d2);
 
@@ -406,7 +477,7 @@ orc_grid* orc_create(const orc_params* p) {
       /* C9: local proper grid spacing ds = min_a |h_a| dx^a */
       double ds = fabs(h[0]) * g->dx[0];
       if (fabs(h[1]) * g->dx[1] < ds) ds = fabs(h[1]) * g->dx[1];
-      if (fabs(h[2]) * g->dx[2] < ds) ds = fabs(h[2]) * g->dx[2];
+      if (!cart && fabs(h[2]) * g->dx[2] < ds) ds = fabs(h[2]) * g->dx[2]; /* C25: x2 part in zds */
       g->ds[q] = ds;
       orc_radial_at(p->coord, p->amp, p->sinhw, p->bscale, g->x0[i0], g->x1[i1], &g->rad0[q],
                     &g->rad1[q], &g->invr[q]);
@@ -419,6 +490,8 @@ orc_grid* orc_create(const orc_params* p) {
       const double ds = g->ds[(size_t)i0 + (size_t)g->T[0] * (size_t)i1];
       if (ds < dsmin) dsmin = ds;
     }
+  for (int i2 = ng; i2 < p->n[2] + ng; ++i2) /* C25: the x2 spacing takes part in the minimum */
+    if (g->zds[i2] < dsmin) dsmin = g->zds[i2];
   g->dsmin = dsmin;
   g->dt = p->cfl * dsmin;
   for (size_t q = 0; q < np; ++q) g->c[q] = p->c_min * g->ds[q] / dsmin;
@@ -473,6 +546,14 @@ void orc_destroy(orc_grid* g) {
   free(g->rad0);
   free(g->rad1);
   free(g->invr);
+  free(g->z22);
+  free(g->z2);
+  free(g->zds);
+  free(g->zh);
+  for (int a = 0; a < 3; ++a) {
+    free(g->X[a]);
+    free(g->ih[a]);
+  }
   free(g->inner_dst);
   free(g->inner_src);
   free(g->outer_idx);
@@ -507,6 +588,14 @@ void orc_get_bc_lists(const orc_grid* g, int32_t* inner_dst, int32_t* inner_src,
 }
 
 double orc_bc_max_frac_err(const orc_grid* g) { return g->bc_max_frac_err; }
+
+void orc_get_axis2(const orc_grid* g, double* z22, double* z2, double* zds, double* zh) {
+  const size_t nb = sizeof(double) * (size_t)g->T[2];
+  if (z22) memcpy(z22, g->z22, nb);
+  if (z2) memcpy(z2, g->z2, nb);
+  if (zds) memcpy(zds, g->zds, nb);
+  if (zh) memcpy(zh, g->zh, nb);
+}
 
 void orc_get_source(const orc_grid* g, double* psi, double* S) {
   if (psi) memcpy(psi, g->psi, sizeof(double) * (size_t)g->ntot);

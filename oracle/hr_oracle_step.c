@@ -53,6 +53,14 @@ static real FN(orc_lap_point)(const orc_grid* g, const real* u, int i0, int i1, 
   d11 *= idxx1;
   d22 *= idxx2;
   const size_t q = (size_t)i0 + (size_t)g->T[0] * (size_t)i1;
+  if (g->p.coord == ORC_SINHCARTESIAN) {
+    /* C25: the u_22 factor depends on x2 and there is a u_2 term (sum_a [u_aa/h_a^2 - X_a''/X_a'^3 u_a]) */
+    real d2 = 0;
+    for (int k = 1; k <= n; ++k) d2 += (real)g->c1[k] * (u[c + k * s2] - u[c - k * s2]);
+    d2 *= (real)(1.0 / g->dx[2]);
+    return (real)g->g00[q] * d00 + (real)g->g11[q] * d11 + (real)g->z22[i2] * d22 +
+           (real)g->g0[q] * d0 + (real)g->g1[q] * d1 + (real)g->z2[i2] * d2;
+  }
   return (real)g->g00[q] * d00 + (real)g->g11[q] * d11 + (real)g->g22[q] * d22 +
          (real)g->g0[q] * d0 + (real)g->g1[q] * d1;
 }
@@ -77,7 +85,7 @@ void FN(orc_rhs_interior)(const orc_grid* g, const real* u, const real* v, real*
     for (int i1 = ng; i1 < g->p.n[1] + ng; ++i1)
       for (int i0 = ng; i0 < g->p.n[0] + ng; ++i0) {
         const int64_t c = orc_idx(g, i0, i1, i2);
-        const real cw = (real)g->c[(size_t)i0 + (size_t)g->T[0] * (size_t)i1];
+        const real cw = (real)orc_c_at(g, (size_t)i0 + (size_t)g->T[0] * (size_t)i1, i2);
         const real lap = FN(orc_lap_point)(g, u, i0, i1, i2);
         const real src = (real)g->S[c] * FN(orc_pow_m7)((real)g->psi[c] + u[c]);
         ku[c] = v[c] - eta * u[c];
@@ -91,7 +99,51 @@ void FN(orc_rhs_interior)(const orc_grid* g, const real* u, const real* v, real*
  *   along an axis in which the point lies beyond the interior (backward on the high side, forward
  *   on the low side), centred otherwise.  SinhSpherical / SinhSymTP outer points lie beyond x0 only
  *   (backward d_0, centred d_1); SinhCylindrical ones (C24) also beyond either end of x1.        */
+/* C25 (SinhCartesian): every ghost point is an outer point; r = |X|, d_r f = sum_a (X_a / r) (1/h_a) d_a f
+ * over the three axes, the same one-sided / centred rule per axis; c from orc_c_at.                  */
+static void FN(orc_bc_outer_cart)(const orc_grid* g, const real* u, const real* v, real* ku, real* kv) {
+  const int64_t st[3] = {1, g->T[0], (int64_t)g->T[0] * g->T[1]};
+#pragma omp parallel for schedule(static)
+  for (int64_t m = 0; m < g->n_outer; ++m) {
+    const int64_t c = g->outer_idx[m];
+    int i[3];
+    i[0] = (int)(c % g->T[0]);
+    i[1] = (int)((c / g->T[0]) % g->T[1]);
+    i[2] = (int)(c / ((int64_t)g->T[0] * g->T[1]));
+    const double X0 = g->X[0][i[0]], X1 = g->X[1][i[1]], X2 = g->X[2][i[2]];
+    const double dist = sqrt(X0 * X0 + X1 * X1 + X2 * X2);
+    const real cw = (real)orc_c_at(g, (size_t)i[0] + (size_t)g->T[0] * (size_t)i[1], i[2]);
+    const real ir = (real)(1.0 / dist);
+    real rad[3], hh[3];
+    for (int a = 0; a < 3; ++a) {
+      rad[a] = (real)(g->X[a][i[a]] * g->ih[a][i[a]] / dist);
+      hh[a] = (real)(1.0 / (2.0 * g->dx[a]));
+    }
+    const real* f[2] = {u, v};
+    real* k[2] = {ku, kv};
+    for (int b = 0; b < 2; ++b) {
+      real acc = 0;
+      for (int a = 0; a < 3; ++a) {
+        const int64_t s = st[a];
+        real d;
+        if (i[a] >= g->p.n[a] + g->ng)
+          d = ((real)3 * f[b][c] - (real)4 * f[b][c - s] + f[b][c - 2 * s]) * hh[a];
+        else if (i[a] < g->ng)
+          d = ((real)4 * f[b][c + s] - (real)3 * f[b][c] - f[b][c + 2 * s]) * hh[a];
+        else
+          d = (f[b][c + s] - f[b][c - s]) * hh[a];
+        acc += rad[a] * d;
+      }
+      k[b][c] = -cw * (acc + f[b][c] * ir);
+    }
+  }
+}
+
 void FN(orc_bc_outer)(const orc_grid* g, const real* u, const real* v, real* ku, real* kv) {
+  if (g->p.coord == ORC_SINHCARTESIAN) {
+    FN(orc_bc_outer_cart)(g, u, v, ku, kv);
+    return;
+  }
   const int64_t s1 = g->T[0];
   const real h0 = (real)(1.0 / (2.0 * g->dx[0])), h1 = (real)(1.0 / (2.0 * g->dx[1]));
 #pragma omp parallel for schedule(static)
@@ -193,7 +245,8 @@ void FN(orc_residual)(const orc_grid* g, const real* u, int32_t mode, double* ou
         const real lap = FN(orc_lap_point)(g, u, i0, i1, i2);
         const real h = lap + (real)g->S[c] * FN(orc_pow_m7)((real)g->psi[c] + u[c]);
         if (H) H[c] = h;
-        const double w = (mode == 0) ? g->w[(size_t)i0 + (size_t)g->T[0] * (size_t)i1] : 1.0;
+        /* C16 weight |h0 h1 h2| (C25: the plane holds |h0 h1|, zh the x2 factor; zh = 1 otherwise) */
+        const double w = (mode == 0) ? g->w[(size_t)i0 + (size_t)g->T[0] * (size_t)i1] * g->zh[i2] : 1.0;
         a += w * (double)h * (double)h;
         b += w;
       }
