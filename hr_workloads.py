@@ -76,7 +76,7 @@ def random_punctures(seed: int, count: int = 2) -> list:
 
 def sweep_point(index: int, n, coord: str, fd_order: int) -> dict:
     """One point of configs[4]'s throughput sweep (grid x coordinate system x FD order)."""
-    if coord in ("SinhSpherical", "SinhCylindrical"):  # cylindrical-like (C24): same amplitude and width
+    if coord in ("SinhSpherical", "SinhCylindrical", "SinhCartesian"):  # C24, C25: same amplitude and width
         geo = dict(amp=1.0e4, sinhw=0.2)
     else:
         geo = dict(amp=1.0e6, sinhw=0.07, bscale=5.0)

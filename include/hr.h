@@ -53,8 +53,10 @@ typedef enum {
 /* Reference metrics ("Cartesian-like, spherical-like, cylindrical-like, and bispherical-like"):
  * SinhSpherical and SinhSymTP (reading C4: x0 in [0,1], x1 = theta in [0,pi], x2 = phi) and SinhCylindrical
  * (reading C24: x0 in [0,1] -> R = rho(x0), x1 in [-1,1] -> Z = rho(x1), same amp and sinhw, x2 = phi; outer
- * points beyond the outer cylinder AND beyond both end faces; default and running-sum arrangements only). */
-typedef enum { HR_SINHSPHERICAL = 0, HR_SINHSYMTP = 1, HR_SINHCYLINDRICAL = 2 } hr_coord;
+ * points beyond the outer cylinder AND beyond both end faces) and SinhCartesian (reading C25: x^a in [-1,1],
+ * X_a = rho(x^a) on every axis; a u_2 term, factors that depend on x2, every ghost point an outer point, no inner
+ * points).  The last two run in the default and running-sum arrangements (variant 0, 3) only. */
+typedef enum { HR_SINHSPHERICAL = 0, HR_SINHSYMTP = 1, HR_SINHCYLINDRICAL = 2, HR_SINHCARTESIAN = 3 } hr_coord;
 typedef enum { HR_F64 = 0, HR_F32 = 1 } hr_dtype;                 /* reading C19           */
 
 /* One Brandt-Bruegmann puncture: bare mass, Cartesian position, Bowen-York

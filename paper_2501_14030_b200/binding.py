@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, os.path.basename(os.environ.get("HR_B200_LIB", "libhr_b200.so")))
 
 HR_OK = 0
-HR_SINHSPHERICAL, HR_SINHSYMTP, HR_SINHCYLINDRICAL = 0, 1, 2
+HR_SINHSPHERICAL, HR_SINHSYMTP, HR_SINHCYLINDRICAL, HR_SINHCARTESIAN = 0, 1, 2, 3
 HR_F64, HR_F32 = 0, 1
 _STATUS = {0: "HR_OK", 1: "HR_ERR_INVALID_ARG", 2: "HR_ERR_UNSUPPORTED", 3: "HR_ERR_WORKSPACE",
            4: "HR_ERR_CUDA", 5: "HR_ERR_NUMERIC"}
@@ -147,7 +147,7 @@ def make_params(params: dict, dtype="f64", device=0, stream=0, residual_mode=0, 
     p = hr_params()
     p.n[:] = [int(x) for x in params["n"]]
     p.coord = {"SinhSpherical": HR_SINHSPHERICAL, "SinhSymTP": HR_SINHSYMTP,
-               "SinhCylindrical": HR_SINHCYLINDRICAL}[params["coord"]]
+               "SinhCylindrical": HR_SINHCYLINDRICAL, "SinhCartesian": HR_SINHCARTESIAN}[params["coord"]]
     p.fd_order = int(params["fd_order"])
     p.dtype = {"f64": HR_F64, "f32": HR_F32}[dtype]
     p.amp = float(params["amp"])

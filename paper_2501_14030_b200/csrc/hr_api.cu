@@ -51,14 +51,15 @@ hr_status validate(const hr_params* p) {
   if (!p) return fail(HR_ERR_INVALID_ARG, "params is NULL");
   if (p->fd_order % 2 != 0 || p->fd_order < 2 || p->fd_order > 2 * HR_MAX_NG)
     return fail(HR_ERR_UNSUPPORTED, "fd_order %d not in {2,4,...,%d}", p->fd_order, 2 * HR_MAX_NG);
-  if (p->coord != HR_SINHSPHERICAL && p->coord != HR_SINHSYMTP && p->coord != HR_SINHCYLINDRICAL)
+  if (p->coord < HR_SINHSPHERICAL || p->coord > HR_SINHCARTESIAN)
     return fail(HR_ERR_UNSUPPORTED, "coord %d unknown", p->coord);
   if (p->dtype != HR_F64 && p->dtype != HR_F32)
     return fail(HR_ERR_UNSUPPORTED, "dtype %d unknown", p->dtype);
   if (p->variant < 0 || p->variant > 3)
     return fail(HR_ERR_UNSUPPORTED, "variant %d unknown", p->variant);
-  if (p->coord == HR_SINHCYLINDRICAL && (p->variant == 1 || p->variant == 2))
-    return fail(HR_ERR_UNSUPPORTED, "SinhCylindrical runs in the marching arrangements (variant 0 or 3) only");
+  if ((p->coord == HR_SINHCYLINDRICAL || p->coord == HR_SINHCARTESIAN) && (p->variant == 1 || p->variant == 2))
+    return fail(HR_ERR_UNSUPPORTED,
+                "SinhCylindrical / SinhCartesian run in the marching arrangements (variant 0 or 3) only");
   const int ng = p->fd_order / 2;
   for (int a = 0; a < 3; ++a)
     if (p->n[a] < ng)
@@ -90,7 +91,8 @@ struct Layout {
   size_t off_field[10];
   size_t off_plane[6];
   size_t off_rad[3];
-  size_t off_opos;
+  size_t off_opos, off_zax[3], off_zh, off_ax;
+  int axs;
   size_t off_wvol, off_inner_dst, off_inner_src, off_partials, off_result, off_counters;
   size_t off_rho, off_rhoz, off_sinth, off_costh, off_sinph, off_cosph, off_punct;
   size_t total;
@@ -105,9 +107,10 @@ Layout make_layout(const hr_params* p) {
   for (int a = 0; a < 3; ++a) L.T[a] = p->n[a] + 2 * L.ng;
   L.ntot = (int64_t)L.T[0] * L.T[1] * L.T[2];
   // outer points (C13): NG layers beyond x0 at interior angles; C24: beyond the cylinder (all x1) and both ends
-  const int64_t n_outer = p->coord == HR_SINHCYLINDRICAL
-                              ? ((int64_t)L.ng * L.T[1] + 2 * (int64_t)L.ng * p->n[0]) * p->n[2]
-                              : (int64_t)L.ng * p->n[1] * p->n[2];
+  int64_t n_outer = p->coord == HR_SINHCYLINDRICAL
+                        ? ((int64_t)L.ng * L.T[1] + 2 * (int64_t)L.ng * p->n[0]) * p->n[2]
+                        : (int64_t)L.ng * p->n[1] * p->n[2];
+  if (p->coord == HR_SINHCARTESIAN) n_outer = L.ntot - (int64_t)p->n[0] * p->n[1] * p->n[2];  // C25: all ghosts
   L.n_inner = L.ntot - (int64_t)p->n[0] * p->n[1] * p->n[2] - n_outer;
   const size_t w = p->dtype == HR_F64 ? 8 : 4;
   hrk_row_geometry(L.T[0], L.ng, w, &L.P0, &L.off0);
@@ -125,6 +128,10 @@ Layout make_layout(const hr_params* p) {
   const size_t n_o2_max = (size_t)L.ng * L.T[1] + 2 * (size_t)L.ng * L.T[0];
   for (int f = 0; f < 3; ++f) L.off_rad[f] = take(n_o2_max * w);
   L.off_opos = take(n_o2_max * 4);
+  L.axs = std::max(L.T[0], std::max(L.T[1], L.T[2]));
+  for (int f = 0; f < 3; ++f) L.off_zax[f] = take((size_t)L.T[2] * w);
+  L.off_zh = take((size_t)L.T[2] * 8);
+  L.off_ax = take((size_t)9 * L.axs * w);
   L.off_wvol = take(np * 8);
   L.off_inner_dst = take((size_t)L.n_inner * 4 + 4);
   L.off_inner_src = take((size_t)L.n_inner * 4 + 4);
@@ -169,7 +176,18 @@ Radial radial_map(const hr_params& p, double x0) {
 MetricPoint metric_point(const hr_params& p, const Radial& R, double sth, double cth, const Radial& Z) {
   MetricPoint m;
   const double A = R.f, A1 = R.d1, A2 = R.d2;
-  if (p.coord == HR_SINHCYLINDRICAL) {
+  if (p.coord == HR_SINHCARTESIAN) {
+    // C25: h_a = X_a'; the x2 parts (h2, the u_22 and u_2 factors) are per-plane tables, not plane entries
+    m.h0 = A1;
+    m.h1 = Z.d1;
+    m.h2 = std::numeric_limits<double>::infinity();  // takes no part in the plane's spacing minimum
+    m.g00 = 1.0 / (A1 * A1);
+    m.g11 = 1.0 / (Z.d1 * Z.d1);
+    m.g22 = 1.0;
+    m.g0 = -A2 / (A1 * A1 * A1);
+    m.g1 = -Z.d2 / (Z.d1 * Z.d1 * Z.d1);
+    m.rad0 = m.rad1 = m.invr = 0.0;  // the radiation factors depend on all three coordinates: in-kernel
+  } else if (p.coord == HR_SINHCYLINDRICAL) {
     // flat metric in cylindrical coordinates (R(x0), Z(x1), phi): h = (R', Z', R)
     m.h0 = A1;
     m.h1 = Z.d1;
@@ -281,6 +299,9 @@ struct HostSetup {
   // of x1, backward d_1; 4: beyond the low end of x1, forward d_1; centred otherwise) and their factors
   std::vector<int32_t> opos;
   std::vector<double> o_r0, o_r1, o_ri;
+  // C25: per-plane tables (T2 each) and the nine per-axis tables of the six-face radiation condition
+  std::vector<double> z22, z2, zc2, zh, ax;
+  int axs = 0;
   std::vector<int32_t> inner_dst, inner_src, outer_idx;
 };
 
@@ -290,27 +311,29 @@ hr_status host_setup(const hr_params* p, HostSetup& H) {
   const int T0 = H.T[0], T1 = H.T[1], T2 = H.T[2];
   const int n0 = p->n[0], n1 = p->n[1], n2 = p->n[2];
   // ---- Alg. 1 l.2: cell-centred coordinate tables (C8) ----
+  const bool cart = p->coord == HR_SINHCARTESIAN;
   const bool cyl = p->coord == HR_SINHCYLINDRICAL;
-  H.dx[0] = 1.0 / n0;
-  H.dx[1] = (cyl ? 2.0 : kPi) / n1;
-  H.dx[2] = 2.0 * kPi / n2;
+  H.dx[0] = (cart ? 2.0 : 1.0) / n0;
+  H.dx[1] = ((cyl || cart) ? 2.0 : kPi) / n1;
+  H.dx[2] = (cart ? 2.0 : 2.0 * kPi) / n2;
   if ((int64_t)T0 * T1 >= (1 << 28)) return fail(HR_ERR_INVALID_ARG, "T0 * T1 exceeds 2^28");
   std::vector<Radial> R(T0), Zt(T1);
   H.rho.resize(T0); H.rhoz.resize(T0); H.sth.resize(T1); H.cth.resize(T1); H.sph.resize(T2);
   H.cph.resize(T2);
   for (int i = 0; i < T0; ++i) {
-    R[i] = radial_map(*p, (i - ng + 0.5) * H.dx[0]);
+    R[i] = radial_map(*p, (cart ? -1.0 : 0.0) + (i - ng + 0.5) * H.dx[0]);
     H.rho[i] = R[i].f;
     H.rhoz[i] =
         p->coord == HR_SINHSYMTP ? std::sqrt(R[i].f * R[i].f + p->bscale * p->bscale) : R[i].f;
     if (cyl) H.rhoz[i] = 1.0;  // the source kernel forms z = rhoz[i0] * costh[i1]: here z = Z(x1)
+    // (C25: the source kernel takes (x, y, z) = (rho[i0], costh[i1], cosph[i2]))
   }
   for (int i = 0; i < T1; ++i) {
     const double th = (i - ng + 0.5) * H.dx[1];
     H.sth[i] = std::sin(th);
     H.cth[i] = std::cos(th);
     Zt[i] = Radial{0.0, 0.0, 0.0};
-    if (cyl) {  // x1 in [-1,1]; (x, y, z) = (R cos phi, R sin phi, Z)
+    if (cyl || cart) {  // x1 in [-1,1]; (x, y, z) = (R cos phi, R sin phi, Z) or (X0, X1, X2)
       Zt[i] = radial_map(*p, -1.0 + (i - ng + 0.5) * H.dx[1]);
       H.sth[i] = 1.0;
       H.cth[i] = Zt[i].f;
@@ -321,6 +344,13 @@ hr_status host_setup(const hr_params* p, HostSetup& H) {
     H.sph[i] = std::sin(ph);
     H.cph[i] = std::cos(ph);
   }
+  std::vector<Radial> X2t(T2);
+  if (cart)
+    for (int i = 0; i < T2; ++i) {
+      X2t[i] = radial_map(*p, -1.0 + (i - ng + 0.5) * H.dx[2]);
+      H.sph[i] = 0.0;
+      H.cph[i] = X2t[i].f;
+    }
 
   // ---- Alg. 1 l.3: reference-metric factor planes, wave speed, dt (C4, C9, C13, C16) ----
   const size_t np = (size_t)T0 * T1;
@@ -336,10 +366,12 @@ hr_status host_setup(const hr_params* p, HostSetup& H) {
       const double d = std::fmin(std::fabs(m.h0) * H.dx[0],
                                  std::fmin(std::fabs(m.h1) * H.dx[1], std::fabs(m.h2) * H.dx[2]));
       ds[q] = d;
-      H.wv[q] = std::fabs(m.h0 * m.h1 * m.h2);
+      H.wv[q] = std::fabs(m.h0 * m.h1 * (cart ? 1.0 : m.h2));  // C25: the x2 factor is the ZH table
       const bool interior = i0 >= ng && i0 < n0 + ng && i1 >= ng && i1 < n1 + ng;
       if (interior && d < dsmin) dsmin = d;
     }
+  if (cart)  // C25: the x2 spacing h2 dx2 takes part in the minimum
+    for (int i2 = ng; i2 < n2 + ng; ++i2) dsmin = std::fmin(dsmin, std::fabs(X2t[i2].d1) * H.dx[2]);
   H.dsmin = dsmin;
   H.dt = p->cfl * dsmin;
   H.r0.assign((size_t)ng * T1, 0.0);
@@ -363,7 +395,7 @@ hr_status host_setup(const hr_params* p, HostSetup& H) {
         H.ri[qo] = c * m.invr;
       }
       const bool in1 = i1 >= ng && i1 < n1 + ng;
-      const bool outer = i0 >= ng && (cyl ? (i0 >= n0 + ng || !in1) : (i0 >= n0 + ng && in1));
+      const bool outer = !cart && i0 >= ng && (cyl ? (i0 >= n0 + ng || !in1) : (i0 >= n0 + ng && in1));
       if (outer) {
         const int bits = (i0 >= n0 + ng ? 1 : 0) | (i1 >= n1 + ng ? 2 : 0) | (i1 < ng ? 4 : 0);
         H.opos.push_back((int32_t)q | (bits << 28));
@@ -373,9 +405,33 @@ hr_status host_setup(const hr_params* p, HostSetup& H) {
       }
     }
 
+  if (cart) {
+    // per-plane tables and the per-axis tables of the radiation condition on the six faces
+    for (auto* v : {&H.z22, &H.z2, &H.zc2, &H.zh}) v->resize((size_t)T2);
+    for (int i = 0; i < T2; ++i) {
+      const double h2 = X2t[i].d1;
+      H.z22[i] = 1.0 / (h2 * h2 * H.dx[2] * H.dx[2]);
+      H.z2[i] = -X2t[i].d2 / (h2 * h2 * h2) / H.dx[2];
+      const double c = p->c_min * std::fabs(h2) * H.dx[2] / dsmin;
+      H.zc2[i] = c * c;
+      H.zh[i] = h2;
+    }
+    H.axs = std::max(T0, std::max(T1, T2));
+    H.ax.assign((size_t)9 * H.axs, 0.0);
+    const std::vector<Radial>* tabs[3] = {&R, &Zt, &X2t};
+    const int Ta[3] = {T0, T1, T2};
+    for (int a = 0; a < 3; ++a)
+      for (int i = 0; i < Ta[a]; ++i) {
+        const Radial& r = (*tabs[a])[i];
+        H.ax[(size_t)(3 * a + 0) * H.axs + i] = r.f;
+        H.ax[(size_t)(3 * a + 1) * H.axs + i] = 1.0 / (2.0 * H.dx[a] * r.d1);
+        H.ax[(size_t)(3 * a + 2) * H.axs + i] = p->c_min * std::fabs(r.d1) * H.dx[a] / dsmin;
+      }
+  }
+
   // ---- Alg. 1 l.4: boundary containers (C13, C14), ascending destination index ----
   const int64_t ntot = (int64_t)T0 * T1 * T2;
-  const int64_t n_outer = (int64_t)H.opos.size() * n2;
+  const int64_t n_outer = cart ? ntot - (int64_t)n0 * n1 * n2 : (int64_t)H.opos.size() * n2;
   const int64_t n_inner = ntot - (int64_t)n0 * n1 * n2 - n_outer;
   H.inner_dst.reserve((size_t)n_inner);
   H.inner_src.reserve((size_t)n_inner);
@@ -386,7 +442,7 @@ hr_status host_setup(const hr_params* p, HostSetup& H) {
       for (int i0 = 0; i0 < T0; ++i0) {
         const bool in0 = i0 >= ng && i0 < n0 + ng;
         if (in0 && in1 && in2) continue;  // interior
-        if (in2 && i0 >= ng && (cyl ? (i0 >= n0 + ng || !in1) : (i0 >= n0 + ng && in1))) {
+        if (cart || (in2 && i0 >= ng && (cyl ? (i0 >= n0 + ng || !in1) : (i0 >= n0 + ng && in1)))) {
           H.outer_idx.push_back(i0 + T0 * (i1 + T1 * i2));
           continue;  // outer
         }
@@ -481,6 +537,10 @@ hr_status hr_create(const hr_params* p, void* workspace_dev, size_t workspace_by
   a.L0 = base + L.off_plane[3];  a.L1 = base + L.off_plane[4];  a.C2 = base + L.off_plane[5];
   a.RAD0 = base + L.off_rad[0]; a.RAD1 = base + L.off_rad[1]; a.RADI = base + L.off_rad[2];
   a.OPOS = reinterpret_cast<int32_t*>(base + L.off_opos);
+  a.Z22 = base + L.off_zax[0]; a.Z2 = base + L.off_zax[1]; a.ZC2 = base + L.off_zax[2];
+  a.ZH = reinterpret_cast<double*>(base + L.off_zh);
+  a.AX = base + L.off_ax;
+  a.AXS = L.axs;
   a.Wvol = reinterpret_cast<double*>(base + L.off_wvol);
   a.inner_dst = reinterpret_cast<int32_t*>(base + L.off_inner_dst);
   a.inner_src = reinterpret_cast<int32_t*>(base + L.off_inner_src);
@@ -526,6 +586,13 @@ hr_status hr_create(const hr_params* p, void* workspace_dev, size_t workspace_by
   HR_TRY(upload_plane(s, a.RAD1, H.o_r1));
   HR_TRY(upload_plane(s, a.RADI, H.o_ri));
   HR_TRY(upload(a.OPOS, H.opos.data(), H.opos.size() * 4, s->stream));
+  if (p->coord == HR_SINHCARTESIAN) {
+    HR_TRY(upload_plane(s, a.Z22, H.z22));
+    HR_TRY(upload_plane(s, a.Z2, H.z2));
+    HR_TRY(upload_plane(s, a.ZC2, H.zc2));
+    HR_TRY(upload(a.ZH, H.zh.data(), H.zh.size() * 8, s->stream));
+    HR_TRY(upload_plane(s, a.AX, H.ax));
+  }
   s->n_outer = (int64_t)s->outer_idx.size();
   s->g.n_o2 = (int32_t)H.opos.size();
   HR_TRY(upload(a.Wvol, H.wv.data(), np * 8, s->stream));

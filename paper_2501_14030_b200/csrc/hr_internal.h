@@ -56,6 +56,12 @@ struct HrArrays {
   // the outer positions themselves: i0 + T0 i1 in the low 28 bits, stencil bits above (hr_api.cu: HostSetup::opos);
   // RAD0 / RAD1 / RADI are indexed like this list
   int32_t* OPOS;
+  // SinhCartesian (C25) only.  Per plane i2 (T2 each): Z22 = 1/(h2 dx2)^2, Z2 = -X2''/X2'^3 / dx2, ZC2 =
+  // (c_min h2 dx2 / ds_min)^2 in the working dtype, ZH = h2 in fp64.  AX: nine tables of AXS scalars (working
+  // dtype), for a = 0, 1, 2: X_a(i), 1/(2 dx_a h_a(i)), c_min h_a(i) dx_a / ds_min (radiation on six faces).
+  void *Z22, *Z2, *ZC2, *AX;
+  double* ZH;
+  int32_t AXS;
   double* Wvol;  // |h0 h1 h2| plane, always fp64 (C16)
   int32_t* inner_dst;
   int32_t* inner_src;
@@ -136,6 +142,7 @@ struct MarchPlan {
   int gt;        // tiles per group (whole tile rows); items are chunk-major within a group
   int* counters; // device: {next item, CTAs done} per stage kernel, zero between launches
   int sph;       // 1 = SinhSpherical inner map (theta -> pi - theta under rho -> -rho)
+  int cart;      // 1 = SinhCartesian (C25): u_2 term, x2-dependent factors, six outer faces, no images
   int cyl;       // 1 = SinhCylindrical (C24): x1 is axial, no theta reflections, outer points beyond its ends
   int* flag;     // device: set non-zero by a kernel that meets psi_BL + u <= 0 or NaN at an interior point
 };

@@ -64,6 +64,8 @@ struct StepArgs {
   const T *L00, *L11, *L22, *L0, *L1, *C2;
   const T *RAD0, *RAD1, *RADI;
   const int32_t* OPOS;  // outer positions of the (i0,i1) plane with their stencil bits (C13)
+  const T *Z22, *Z2, *ZC2, *AX;  // SinhCartesian (C25): per-plane factors and per-axis radiation tables
+  int AXS;
   T eta;
   T dt;
 };
@@ -372,7 +374,7 @@ __global__ void __launch_bounds__(256)
              const double* __restrict__ costh, const double* __restrict__ sinph,
              const double* __restrict__ cosph, const double* __restrict__ punct, int npunct,
              double ox, double oy, double oz, T* __restrict__ psi_out, T* __restrict__ S_out,
-             int* __restrict__ bad_flag) {
+             int* __restrict__ bad_flag, int cart) {
   const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= g.ntot) return;
   const int i0 = (int)(c % g.T0);
@@ -381,9 +383,10 @@ __global__ void __launch_bounds__(256)
   const int64_t cs = g.off0 + i0 + g.s1 * i1 + g.s2 * i2;  // stored index
   // grid point in Cartesian coordinates (C4) + grid centre (C6)
   const double rs = rho[i0] * sinth[i1];
-  const double x = rs * cosph[i2] + ox;
-  const double y = rs * sinph[i2] + oy;
-  const double z = rhoz[i0] * costh[i1] + oz;
+  // (C25, SinhCartesian: the three tables hold X0(i0), X1(i1), X2(i2))
+  const double x = (cart ? rho[i0] : rs * cosph[i2]) + ox;
+  const double y = (cart ? costh[i1] : rs * sinph[i2]) + oy;
+  const double z = (cart ? cosph[i2] : rhoz[i0] * costh[i1]) + oz;
   double psi = 1.0;
   double axx = 0, ayy = 0, azz = 0, axy = 0, axz = 0, ayz = 0;
   for (int p = 0; p < npunct; ++p) {
@@ -490,6 +493,7 @@ StepArgs<T> make_args(const hr_solver* s, int stage, void* ku, void* kv) {
   r.L00 = P(a.L00); r.L11 = P(a.L11); r.L22 = P(a.L22); r.L0 = P(a.L0); r.L1 = P(a.L1);
   r.C2 = P(a.C2); r.RAD0 = P(a.RAD0); r.RAD1 = P(a.RAD1); r.RADI = P(a.RADI);
   r.OPOS = a.OPOS;
+  r.Z22 = P(a.Z22); r.Z2 = P(a.Z2); r.ZC2 = P(a.ZC2); r.AX = P(a.AX); r.AXS = a.AXS;
   r.eta = (T)s->p.eta;
   r.dt = (T)s->dt;
   return r;
@@ -611,8 +615,8 @@ struct LeanCode {
   static constexpr int S2 = PREC ? 22 : 12, S4 = PREC ? 24 : 14;
 };
 
-#define HR_MARCH_KERNEL(T, NG, STAGE) \
-  k_march<T, NG, STAGE, MarchCfg<T>::TW, MarchCfg<T>::BY, MarchCfg<T>::VX, march_depth<T, STAGE>()>
+#define HR_MARCH_KERNEL(T, NG, STAGE, CART) \
+  k_march<T, NG, STAGE, MarchCfg<T>::TW, MarchCfg<T>::BY, MarchCfg<T>::VX, march_depth<T, STAGE>(), CART>
 #define HR_MARCH_SMEM(T, NG, STAGE) \
   march_smem_bytes<T, NG, STAGE, MarchCfg<T>::TW, MarchCfg<T>::BY, march_depth<T, STAGE>()>()
 
@@ -687,7 +691,7 @@ static void choose_chunks(MarchPlan& m, int n2, int ng, int slots, bool f64) {
 template <typename T, int NG, int STAGE>
 cudaError_t prepare_march_stage(const hr_solver* s, int* grid_out) {
   using C = MarchCfg<T>;
-  auto kern = HR_MARCH_KERNEL(T, NG, STAGE);
+  auto kern = s->plan.cart ? HR_MARCH_KERNEL(T, NG, STAGE, true) : HR_MARCH_KERNEL(T, NG, STAGE, false);
   constexpr size_t smem = HR_MARCH_SMEM(T, NG, STAGE);
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
@@ -783,7 +787,10 @@ cudaError_t launch_march_stage(const hr_solver* s, const StepArgs<T>& a, const R
   const dim3 block(C::TW / C::VX, C::BY, 1);
   const dim3 grid(STAGE >= 10 ? s->march_grid_lean[STAGE % 10] : s->march_grid[STAGE], 1, 1);
   const MarchMaps mm = make_maps(s, STAGE);
-  HR_MARCH_KERNEL(T, NG, STAGE)<<<grid, block, smem, s->stream>>>(s->g, a, s->plan, ra, mm);
+  if (s->plan.cart)
+    HR_MARCH_KERNEL(T, NG, STAGE, true)<<<grid, block, smem, s->stream>>>(s->g, a, s->plan, ra, mm);
+  else
+    HR_MARCH_KERNEL(T, NG, STAGE, false)<<<grid, block, smem, s->stream>>>(s->g, a, s->plan, ra, mm);
   return cudaGetLastError();
 }
 
@@ -793,7 +800,7 @@ cudaError_t launch_march(const hr_solver* s, int stage, void* ku, void* kv, int 
   if (stage == 12) stage = LeanCode<T>::S2;
   if (stage == 14) stage = LeanCode<T>::S4;
   const StepArgs<T> a = make_args<T>(s, stage, ku, kv);
-  const ResidArgs ra{s->a.Wvol, partials, mode, out2};
+  const ResidArgs ra{s->a.Wvol, partials, mode, out2, s->a.ZH};
   switch (stage) {
     case 0: return launch_march_stage<T, NG, 0>(s, a, ra);
     case 1: return launch_march_stage<T, NG, 1>(s, a, ra);
@@ -910,6 +917,7 @@ MarchPlan hrk_make_plan(const int32_t n[3], int ng, int coord, int dtype) {
   m.nty = (n[1] + by - 1) / by;
   m.sph = coord == HR_SINHSPHERICAL ? 1 : 0;
   m.cyl = coord == HR_SINHCYLINDRICAL ? 1 : 0;
+  m.cart = coord == HR_SINHCARTESIAN ? 1 : 0;
   m.zc = n[2];
   m.nzc = 1;
   m.gt = m.ntx * m.nty;
@@ -1061,11 +1069,11 @@ cudaError_t hrk_source(const hr_solver* s) {
     k_source<double><<<blocks, 256, 0, s->stream>>>(
         g, a.rho, a.rhoz, a.sinth, a.costh, a.sinph, a.cosph, a.punct, s->p.n_punctures,
         s->p.origin[0], s->p.origin[1], s->p.origin[2], static_cast<double*>(a.psi),
-        static_cast<double*>(a.S), flag);
+        static_cast<double*>(a.S), flag, s->p.coord == HR_SINHCARTESIAN);
   else
     k_source<float><<<blocks, 256, 0, s->stream>>>(
         g, a.rho, a.rhoz, a.sinth, a.costh, a.sinph, a.cosph, a.punct, s->p.n_punctures,
         s->p.origin[0], s->p.origin[1], s->p.origin[2], static_cast<float*>(a.psi),
-        static_cast<float*>(a.S), flag);
+        static_cast<float*>(a.S), flag, s->p.coord == HR_SINHCARTESIAN);
   return cudaGetLastError();
 }

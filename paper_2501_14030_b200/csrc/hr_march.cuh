@@ -36,6 +36,7 @@ struct ResidArgs {
   double* partials;  // 2 doubles per work item
   int mode;
   double* out2;      // { sum w H^2, sum w }, written by the last CTA to finish
+  const double* ZH;  // SinhCartesian (C25): h2 per plane, the x2 factor of the weight
 };
 
 template <typename T, int VX>
@@ -382,7 +383,9 @@ __host__ __device__ constexpr size_t march_smem_bytes() {
 // 6: RK4 stage 1 that also accumulates the residual of its input state -- the bracket of Eq. 5 at
 // the state Y is exactly H of Eq. 4, so Alg. 1 l.9-11 followed by l.12-16 needs no pass of its own.
 // TW x BY points per tile, VX points per thread along i0, D planes of look-ahead.
-template <typename T, int NG, int STAGE, int TW, int BY, int VX, int D>
+// CART: the SinhCartesian (C25) instantiation -- a u_2 term, per-plane factors, six outer faces, no ghost images.
+// A template parameter because even uniform branches on it in the plane loop cost the other systems 4 %.
+template <typename T, int NG, int STAGE, int TW, int BY, int VX, int D, bool CART>
 __global__ void __launch_bounds__((TW / VX) * BY,
                                   sizeof(T) == 8 ? HR_MARCH_MINB_F64 : HR_MARCH_MINB_F32)
     k_march(const __grid_constant__ HrGrid g, const __grid_constant__ StepArgs<T> a,
@@ -432,6 +435,7 @@ __global__ void __launch_bounds__((TW / VX) * BY,
 
   const int lx = threadIdx.x, ly = threadIdx.y;
   const int tid = ly * BXT + lx;
+  constexpr bool is_cart = CART;  // SinhCartesian (C25)
   const int s2 = g.P0 * g.T1;
   const ImgGeom ig{NG, g.n2, g.T1, g.P0, g.off0, plan.sph};
 
@@ -464,18 +468,84 @@ __global__ void __launch_bounds__((TW / VX) * BY,
   // first TMA loads of its first item, so that its load latency hides behind theirs (on L2-resident
   // grids a CTA lives for one short item: anything serial at its end is on the critical path).
   [[maybe_unused]] auto outer_tail = [&]() {
-    const int n_outer = g.n_o2 * g.n2;
+    const int n_outer = is_cart ? g.T0 * g.T1 * g.T2 - g.n0 * g.n1 * g.n2 : g.n_o2 * g.n2;
     for (int m = blockIdx.x * NT + tid; m < n_outer; m += gridDim.x * NT) {
-      const int qo = m % g.n_o2;
-      const int i2 = NG + m / g.n_o2;
-      const int po = a.OPOS[qo];
-      const int bits = po >> 28, q = po & 0x0fffffff;
-      const int i1 = q / g.T0, i0 = q - i1 * g.T0;
-      const int c = g.off0 + i0 + g.P0 * i1 + s2 * i2;
-      const T r0 = a.RAD0[qo], r1 = a.RAD1[qo], ri = a.RADI[qo];
-      const T uc = a.in_u[c], vc = a.in_v[c];
-      const T ku = radiation_k(a.in_u, c, g.P0, r0, r1, ri, bits);
-      const T kv = radiation_k(a.in_v, c, g.P0, r0, r1, ri, bits);
+      int i0, i1, i2, c;
+      T uc, vc, ku, kv;
+      if (is_cart) {
+        // C25: every ghost point is an outer point.  Shell enumeration: the 2 NG ghost planes of x2 in full,
+        // then per interior plane the 2 NG ghost rows of x1 in full and the 2 NG ghost columns of x0.
+        const int A = g.T0 * g.T1, ring = A - g.n0 * g.n1, nzg = 2 * NG * A;
+        if (m < nzg) {
+          const int pz = m / A, q = m - pz * A;
+          i2 = pz < NG ? pz : g.n2 + pz;
+          i1 = q / g.T0;
+          i0 = q - i1 * g.T0;
+        } else {
+          const int mm2 = m - nzg, pz = mm2 / ring, r = mm2 - pz * ring;
+          i2 = NG + pz;
+          if (r < 2 * NG * g.T0) {
+            const int pr = r / g.T0;
+            i1 = pr < NG ? pr : g.n1 + pr;
+            i0 = r - pr * g.T0;
+          } else {
+            const int r2 = r - 2 * NG * g.T0, row = r2 / (2 * NG), pc = r2 - row * (2 * NG);
+            i1 = NG + row;
+            i0 = pc < NG ? pc : g.n0 + pc;
+          }
+        }
+        c = g.off0 + i0 + g.P0 * i1 + s2 * i2;
+        // r = |X|, d_r f = sum_a (X_a / r) (1/h_a) d_a f, c = c_min min_a(h_a dx_a) / ds_min, from the nine
+        // per-axis tables {X_a, 1/(2 dx_a h_a), c_min h_a dx_a / ds_min} (C13 on six faces)
+        const int ia[3] = {i0, i1, i2};
+        const int na[3] = {g.n0, g.n1, g.n2};
+        const int sa[3] = {1, g.P0, s2};
+        T X[3], rh[3], cw = T(0);
+#pragma unroll
+        for (int ax = 0; ax < 3; ++ax) {
+          X[ax] = a.AX[(3 * ax + 0) * a.AXS + ia[ax]];
+          rh[ax] = a.AX[(3 * ax + 1) * a.AXS + ia[ax]];
+          const T ca = a.AX[(3 * ax + 2) * a.AXS + ia[ax]];
+          cw = (ax == 0 || ca < cw) ? ca : cw;
+        }
+        const T ir = T(1) / sqrt(X[0] * X[0] + X[1] * X[1] + X[2] * X[2]);
+        uc = a.in_u[c];
+        vc = a.in_v[c];
+        T au = T(0), av = T(0);
+#pragma unroll
+        for (int ax = 0; ax < 3; ++ax) {
+          const int st = sa[ax];
+          T du, dv;
+          if (ia[ax] >= na[ax] + NG) {
+            du = T(3) * uc - T(4) * a.in_u[c - st] + a.in_u[c - 2 * st];
+            dv = T(3) * vc - T(4) * a.in_v[c - st] + a.in_v[c - 2 * st];
+          } else if (ia[ax] < NG) {
+            du = T(4) * a.in_u[c + st] - T(3) * uc - a.in_u[c + 2 * st];
+            dv = T(4) * a.in_v[c + st] - T(3) * vc - a.in_v[c + 2 * st];
+          } else {
+            du = a.in_u[c + st] - a.in_u[c - st];
+            dv = a.in_v[c + st] - a.in_v[c - st];
+          }
+          const T rad = X[ax] * ir * rh[ax];
+          au += rad * du;
+          av += rad * dv;
+        }
+        ku = -cw * (au + uc * ir);
+        kv = -cw * (av + vc * ir);
+      } else {
+        const int qo = m % g.n_o2;
+        i2 = NG + m / g.n_o2;
+        const int po = a.OPOS[qo];
+        const int bits = po >> 28, q = po & 0x0fffffff;
+        i1 = q / g.T0;
+        i0 = q - i1 * g.T0;
+        c = g.off0 + i0 + g.P0 * i1 + s2 * i2;
+        const T r0 = a.RAD0[qo], r1 = a.RAD1[qo], ri = a.RADI[qo];
+        uc = a.in_u[c];
+        vc = a.in_v[c];
+        ku = radiation_k(a.in_u, c, g.P0, r0, r1, ri, bits);
+        kv = radiation_k(a.in_v, c, g.P0, r0, r1, ri, bits);
+      }
       T wu, wv;
       if constexpr (LEAN) {
         T yu = T(0), yv = T(0);
@@ -503,7 +573,7 @@ __global__ void __launch_bounds__((TW / VX) * BY,
       const int cB = (!plan.cyl && i1 < 2 * NG) ? 2 * NG - 1 - i1 : -1;
       const int cC = (!plan.cyl && i1 >= g.n1) ? 2 * (g.n1 + NG) - 1 - i1 : -1;
       const int rr = i0 < 2 * NG ? 2 * NG - 1 - i0 : -1;
-      if (cB >= 0 || cC >= 0 || rr >= 0 || i2 < 2 * NG || i2 >= g.n2)
+      if (!is_cart && (cB >= 0 || cC >= 0 || rr >= 0 || i2 < 2 * NG || i2 >= g.n2))
         scatter_images<T>(ig, a.out_u, a.out_v, wu, wv, i0, i1, i2, rr, cB, cC);
     }
   };
@@ -586,7 +656,7 @@ __global__ void __launch_bounds__((TW / VX) * BY,
         if constexpr (RESID) wq[j] = ra.mode == 0 ? ra.W[q] : 1.0;
         if constexpr (ADVANCE) {
           c2[j] = a.C2[q];
-          inplane_images |= i0 + j < 2 * NG;
+          inplane_images |= !is_cart && i0 + j < 2 * NG;
         }
       }
     }
@@ -645,6 +715,15 @@ __global__ void __launch_bounds__((TW / VX) * BY,
           sl = 0;
           par ^= 1u;
         }
+        // C25 (SinhCartesian): what depends on x2 is uniform over the plane
+        T z22 = T(0), z2v = T(0), zc2 = T(0);
+        double zh = 1.0;
+        if (is_cart) {
+          z22 = a.Z22[z];
+          z2v = a.Z2[z];
+          zc2 = a.ZC2[z];
+          if constexpr (RESID) zh = ra.ZH[z];
+        }
         if (nact > 0) {
           if constexpr (PACKED) {
             HR_W(2 * NG)[0] = *reinterpret_cast<const unsigned long long*>(sb + ST_FRONT * (TW * BY) + so);
@@ -694,6 +773,20 @@ __global__ void __launch_bounds__((TW / VX) * BY,
             lap = f2_fma(l22p, d22, lap);
             lap = f2_fma(l0p, f2_pack(d0s[0], d0s[1]), lap);
             lap = f2_fma(l1p, d1, lap);
+            if (is_cart) {  // C25: the u_22 factor belongs to the plane, and there is a u_2 term
+              F2 d2p = f2_bc(0.f);
+#pragma unroll
+              for (int k = 1; k <= NG; ++k)
+                d2p = f2_fma(f2_bc((float)F::c1(k)),
+                             f2_sub(F2{(unsigned long long)HR_W(NG + k)[0]}, F2{(unsigned long long)HR_W(NG - k)[0]}),
+                             d2p);
+              lap = f2_mul(l00p, f2_pack(d00s[0], d00s[1]));
+              lap = f2_fma(l11p, d11, lap);
+              lap = f2_fma(f2_bc((float)z22), d22, lap);
+              lap = f2_fma(l0p, f2_pack(d0s[0], d0s[1]), lap);
+              lap = f2_fma(l1p, d1, lap);
+              lap = f2_fma(f2_bc((float)z2v), d2p, lap);
+            }
             // (psi + u)^-7: hardware reciprocal seed per lane, Newton step and powers packed
             const F2 x = f2_add(L2(sb + ST_PSI * (TW * BY) + so), uc2);
             float x0, x1, r0, r1;
@@ -736,8 +829,15 @@ __global__ void __launch_bounds__((TW / VX) * BY,
           }
 #pragma unroll
           for (int j = 0; j < VX; ++j) {
-            const T lap = l00[j] * d00[j] + l11[j] * d11[j] + l22[j] * d22[j] + l0[j] * d0[j] +
-                          l1[j] * d1[j];
+            T lap = l00[j] * d00[j] + l11[j] * d11[j] + l22[j] * d22[j] + l0[j] * d0[j] +
+                    l1[j] * d1[j];
+            if (is_cart) {  // C25: the u_22 factor belongs to the plane, and there is a u_2 term
+              T d2 = T(0);
+#pragma unroll
+              for (int k = 1; k <= NG; ++k) d2 += T(F::c1(k)) * (HR_W(NG + k)[j] - HR_W(NG - k)[j]);
+              lap = l00[j] * d00[j] + l11[j] * d11[j] + z22 * d22[j] + l0[j] * d0[j] + l1[j] * d1[j] +
+                    z2v * d2;
+            }
             const T x = psi.v[j] + HR_W(NG)[j];
             bad |= j < nact & !(x > T(0));
             H[j] = lap + Ss.v[j] * pow_m7(x);
@@ -747,8 +847,9 @@ __global__ void __launch_bounds__((TW / VX) * BY,
 #pragma unroll
             for (int j = 0; j < VX; ++j)
               if (j < nact) {
-                num += wq[j] * (double)H[j] * (double)H[j];
-                den += wq[j];
+                const double wj = (is_cart && ra.mode == 0) ? wq[j] * zh : wq[j];
+                num += wj * (double)H[j] * (double)H[j];
+                den += wj;
               }
           }
           if constexpr (ADVANCE) {
@@ -776,7 +877,8 @@ __global__ void __launch_bounds__((TW / VX) * BY,
               };
               const F2 vin2 = L2(sb + ST_V * (TW * BY) + so);
               const F2 ku = f2_fma(f2_bc(-(float)a.eta), uc2, vin2);
-              const F2 kv = f2_mul(c2p, H2);
+              const F2 kv = f2_mul(is_cart ? f2_pack(fminf((float)c2[0], (float)zc2), fminf((float)c2[VX - 1], (float)zc2))
+                                             : c2p, H2);
               F2 yu2{}, yv2{}, au2{}, av2{};
               if constexpr (NEED_A) {
                 au2 = L2(sb + S_AU * (TW * BY) + so);
@@ -814,7 +916,7 @@ __global__ void __launch_bounds__((TW / VX) * BY,
               for (int j = 0; j < VX; ++j) {
                 const T uc = HR_W(NG)[j];
                 const T ku = vin.v[j] - a.eta * uc;
-                const T kv = c2[j] * H[j];
+                const T kv = (is_cart ? (c2[j] < zc2 ? c2[j] : zc2) : c2[j]) * H[j];
                 if constexpr (LEAN) {
                   if constexpr (PREC && RK == 4) {
                     wu.v[j] = rk_prec_4<T>(a.dt, ku, uc, yu.v[j], au.v[j]);
@@ -856,7 +958,7 @@ __global__ void __launch_bounds__((TW / VX) * BY,
                   }
                 }
             }
-            if (inplane_images || z < 2 * NG || z >= g.n2)
+            if (!is_cart && (inplane_images || z < 2 * NG || z >= g.n2))
               scatter_vec<T, VX>(ig, a.out_u, a.out_v, wu, wv, i0, i1, z, nact, cB, cC);
           }
         }

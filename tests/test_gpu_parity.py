@@ -54,6 +54,10 @@ SMALL = [
     ("cyl_o4", W.sweep_point(8, (40, 24, 16), "SinhCylindrical", 4)),
     ("cyl_o8_ragged", W.sweep_point(9, (33, 19, 10), "SinhCylindrical", 8)),
     ("cyl_o10_ragged", W.sweep_point(10, (35, 37, 12), "SinhCylindrical", 10)),
+    # Cartesian-like reference metric (reading C25): u_2 term, x2-dependent factors, six outer faces
+    ("cart_o4", W.sweep_point(11, (40, 24, 16), "SinhCartesian", 4)),
+    ("cart_o8_ragged", W.sweep_point(12, (33, 19, 10), "SinhCartesian", 8)),
+    ("cart_o10_ragged", W.sweep_point(13, (35, 37, 12), "SinhCartesian", 10)),
 ]
 
 
@@ -158,7 +162,9 @@ STEP_CASES = [("config0", W.config(0), 200), ("config1_half", dict(W.config(1, s
               ("sph_o6_ragged", dict(W.sweep_point(0, (70, 18, 10), "SinhSpherical", 6), eta=2.0), 100),
               # (eta dt must stay well below RK4's real-axis limit 2.78, C10: dt = 3.2 and 1.7 on these coarse grids)
               ("cyl_o8_ragged", dict(W.sweep_point(9, (33, 38, 10), "SinhCylindrical", 8), eta=0.2), 100),
-              ("cyl_o4", dict(W.sweep_point(8, (40, 48, 16), "SinhCylindrical", 4), eta=0.2), 200)]
+              ("cyl_o4", dict(W.sweep_point(8, (40, 48, 16), "SinhCylindrical", 4), eta=0.2), 200),
+              ("cart_o8_ragged", dict(W.sweep_point(12, (33, 38, 26), "SinhCartesian", 8), eta=0.02), 100),
+              ("cart_o4", dict(W.sweep_point(11, (40, 48, 32), "SinhCartesian", 4), eta=0.02), 200)]
 
 
 @pytest.mark.parametrize("name,params,steps", STEP_CASES, ids=[c[0] for c in STEP_CASES])

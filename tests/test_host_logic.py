@@ -74,7 +74,9 @@ CASES = [W.config(0), W.config(1), W.config(1, scale=0.3), W.config(3, scale=0.1
          W.sweep_point(2, (7, 5, 6), "SinhSpherical", 10),
          W.sweep_point(3, (16, 4, 4), "SinhSymTP", 2),
          W.sweep_point(4, (12, 10, 8), "SinhCylindrical", 4),   # reading C24
-         W.sweep_point(5, (9, 7, 6), "SinhCylindrical", 10)]
+         W.sweep_point(5, (9, 7, 6), "SinhCylindrical", 10),
+         W.sweep_point(6, (10, 12, 8), "SinhCartesian", 4),     # reading C25
+         W.sweep_point(7, (7, 9, 12), "SinhCartesian", 8)]
 
 
 @pytest.mark.parametrize("params", CASES, ids=lambda p: f"{p['name']}-{p['coord']}-o{p['fd_order']}")
@@ -92,6 +94,8 @@ def test_host_setup_matches_oracle(hr, params):
     pl = o.planes()
     n = params["n"]
     dx = [1.0 / n[0], (2.0 if params["coord"] == "SinhCylindrical" else np.pi) / n[1], 2 * np.pi / n[2]]
+    if params["coord"] == "SinhCartesian":
+        dx = [2.0 / n[0], 2.0 / n[1], 2.0 / n[2]]
     ng = o.ng
     inner = (slice(ng, -ng), slice(ng, -ng))  # factors are only used at interior (i0,i1)
     for name, ref in (("L00", pl["g00"] / dx[0] ** 2), ("L11", pl["g11"] / dx[1] ** 2),
