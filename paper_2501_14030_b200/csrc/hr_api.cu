@@ -1088,7 +1088,9 @@ hr_status hr_query(hr_solver* s, int32_t what, int64_t* value) {
       return HR_OK;
     }
     case HR_Q_PLAN_ZC: *value = s->plan.zc; return HR_OK;
-    case HR_Q_PLAN_ITEMS: *value = (int64_t)s->plan.ntx * s->plan.nty * s->plan.nzc; return HR_OK;
+    case HR_Q_PLAN_ITEMS:  // long items (segments of plan.mseg chunks) + single chunks
+      *value = s->plan.ncol + ((int64_t)s->plan.ntx * s->plan.nty * s->plan.nseg - s->plan.ncol) * s->plan.mseg;
+      return HR_OK;
     case HR_Q_PLAN_GRID: *value = s->p.variant == 0 ? s->march_grid_lean[2] : s->march_grid[2]; return HR_OK;
   }
   return fail(HR_ERR_INVALID_ARG, "unknown query %d", what);

@@ -139,7 +139,12 @@ struct HrArrays {
 struct MarchPlan {
   int ntx, nty;  // tiles along i0, i1
   int zc, nzc;   // planes per chunk, chunks along i2
-  int gt;        // tiles per group (whole tile rows); items are chunk-major within a group
+  int gt;        // tiles per group (whole tile rows); items are chunk-major within a group (unused since r2)
+  // Long items: a tile's column of chunks is cut into nseg segments of mseg chunks; the first ncol segments
+  // (segment-major over the tiles, a whole number of waves of CTAs) are marched in one go -- one window
+  // priming and one pipeline start per segment instead of per chunk -- and the chunks of the remaining
+  // segments are handed out one by one, chunk-major, to even out the end.  ncol = 0, mseg = 1: chunks only.
+  int mseg, nseg, ncol;
   int* counters; // device: {next item, CTAs done} per stage kernel, zero between launches
   int sph;       // 1 = SinhSpherical inner map (theta -> pi - theta under rho -> -rho)
   int cart;      // 1 = SinhCartesian (C25): u_2 term, x2-dependent factors, six outer faces, no images

@@ -921,6 +921,9 @@ MarchPlan hrk_make_plan(const int32_t n[3], int ng, int coord, int dtype) {
   m.zc = n[2];
   m.nzc = 1;
   m.gt = m.ntx * m.nty;
+  m.mseg = 1;
+  m.nseg = 1;
+  m.ncol = 0;
   (void)ng;
   return m;
 }
@@ -931,7 +934,21 @@ void hrk_replan(hr_solver* s, int share) {
   // one chunking for all stages, balanced for the RK stage kernels (stages 2, 3 dominate)
   const int slots = s->march_slots[2] / share > 0 ? s->march_slots[2] / share : 1;
   choose_chunks(s->plan, s->g.n2, s->g.ng, slots, s->p.dtype == HR_F64);
-  const long long items = (long long)s->plan.ntx * s->plan.nty * s->plan.nzc;
+  MarchPlan& m = s->plan;
+  const long long ntiles = (long long)m.ntx * m.nty;
+  m.mseg = 1;
+  m.nseg = m.nzc;
+  m.ncol = 0;
+  const char* col_env = std::getenv("HR_TUNE_COL");  // tuning knob: 0 = chunks only
+  if (!(col_env && std::atoi(col_env) == 0) && ntiles * m.nzc >= 2LL * slots && m.nzc > 1) {
+    long long k = (slots + ntiles - 1) / ntiles;  // segments per tile: at least `slots` long items in all
+    if (k > m.nzc) k = m.nzc;
+    m.mseg = (int)((m.nzc + k - 1) / k);
+    m.nseg = (m.nzc + m.mseg - 1) / m.mseg;
+    m.ncol = (int)((ntiles * m.nseg / slots) * slots);
+    if (m.mseg == 1) m.ncol = 0;
+  }
+  const long long items = m.ncol + (ntiles * m.nseg - m.ncol) * m.mseg;
   for (int st = 0; st < 7; ++st) {
     s->march_grid[st] = (int)std::min<long long>(s->march_slots[st], items);
     s->march_grid_lean[st] = (int)std::min<long long>(s->march_slots_lean[st], items);

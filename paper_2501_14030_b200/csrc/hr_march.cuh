@@ -405,6 +405,9 @@ __global__ void __launch_bounds__((TW / VX) * BY,
   // Y_new = (1/3)(Q + Y3) + dt/6 k4 = Y + dt/6 (k1 + 2 k2 + 2 k3 + k4).  Bytes per point:
   // 6w, 10w, 8w, 8w = 32w per step instead of 8w, 12w, 12w, 8w = 40w.
   constexpr bool LEAN = STAGE >= 10;
+  // the numeric guard (psi_BL + u <= 0 or NaN -> plan.flag) looks at the state a step starts from and at the
+  // residual's / hr_eval_rhs's input: stages 2-4 of a step that goes wrong feed a stage 1 that reports it
+  constexpr bool GUARD = STAGE % 10 == 0 || STAGE % 10 == 1 || STAGE % 10 == 5 || STAGE % 10 == 6;
   constexpr bool PREC = STAGE >= 20;  // increment-preserving stages 22 and 24 (rk_prec_q, rk_prec_4)
   constexpr int ST = STAGE % 10;
   constexpr int RK = ST == 6 ? 1 : ST;                  // which RK combine (0 = store k)
@@ -448,7 +451,9 @@ __global__ void __launch_bounds__((TW / VX) * BY,
 
   // work items = (chunk of planes, tile), chunk-major
   const int ntiles = plan.ntx * plan.nty;
-  const int n_items = ntiles * plan.nzc;
+  const int n_long = ntiles * plan.nseg;                              // segments of plan.mseg chunks
+  const int n_items = plan.ncol + (n_long - plan.ncol) * plan.mseg;   // long items, then single chunks
+  const int n_part = ntiles * plan.nzc;                               // residual partials: one per (tile, chunk)
   // no more items than CTAs (small grids): every CTA has exactly one item, nothing is handed out, and
   // no atomic round trip sits at the end of the CTA's (short) life
   const bool dynamic = n_items > (int)gridDim.x;
@@ -585,24 +590,35 @@ __global__ void __launch_bounds__((TW / VX) * BY,
   __shared__ double red[2][NT / 32];
   int item = blockIdx.x;
   while (item < n_items) {
-    // item -> (group of tile rows, chunk, tile in group): chunk-major inside a group of plan.gt
-    // tiles, so that neighbouring tiles of the same planes run together (halo rows meet in L2)
-    // AND the chunks of a tile follow each other closely enough for the 2NG planes their
-    // windows share to still be in L2
-    const int per_group = plan.gt * plan.nzc;
-    const int grp = item / per_group;
-    const int gt_here = min(plan.gt, ntiles - grp * plan.gt);  // the last group may be smaller
-    const int rem = item - grp * per_group;
-    const int chunk = rem / gt_here;
-    const int tile_id = grp * plan.gt + (rem - chunk * gt_here);
-    const int zi = chunk * plan.zc;
-    const int seg = min(plan.zc, g.n2 - zi);
+    // item -> (tile, first chunk, number of chunks).  The first plan.ncol items are whole segments of
+    // plan.mseg chunks, segment-major over the tiles: neighbouring tiles march up the same planes together
+    // (halo rows meet in L2) and a segment primes its i2 window and starts its TMA pipeline once.  The
+    // chunks of the remaining segments follow one by one, chunk-major, to even out the end of the launch.
+    int tile_id, ch0, nch;
+    if (item < plan.ncol) {
+      const int sgi = item / ntiles;
+      tile_id = item - sgi * ntiles;
+      ch0 = sgi * plan.mseg;
+      nch = min(plan.mseg, plan.nzc - ch0);
+    } else {
+      const int nrem = n_long - plan.ncol;
+      const int rem = item - plan.ncol;
+      const int cpos = rem / nrem;
+      const int sid = plan.ncol + (rem - cpos * nrem);
+      const int sgi = sid / ntiles;
+      tile_id = sid - sgi * ntiles;
+      ch0 = sgi * plan.mseg + cpos;
+      nch = ch0 < plan.nzc ? 1 : 0;  // the last segment of a tile may be shorter: an empty item
+      if (nch == 0) ch0 = 0;
+    }
+    const int zi = ch0 * plan.zc;
+    const int seg = nch > 0 ? min(nch * plan.zc, g.n2 - zi) : 0;
     const int tx = tile_id % plan.ntx, ty = tile_id / plan.ntx;
     const int z_begin = NG + zi, z_end = z_begin + seg;
     const int x0 = NG + tx * TW, y0 = NG + ty * BY;  // first point of the tile
     const int i0 = x0 + VX * lx, i1 = y0 + ly;
     // number of this thread's points that are interior (0..VX)
-    const int nact = i1 < g.n1 + NG ? max(0, min(VX, g.n0 + NG - i0)) : 0;
+    const int nact = (i1 < g.n1 + NG && nch > 0) ? max(0, min(VX, g.n0 + NG - i0)) : 0;
     const int col = g.off0 + i0 + g.P0 * i1;  // only dereferenced if nact > 0
 
     // one thread feeds the ring: everything plane zz needs, into ring slot sl
@@ -699,7 +715,35 @@ __global__ void __launch_bounds__((TW / VX) * BY,
     const int so = ly * TW + VX * lx;                                     // in a TW x BY box
     const int to = (ly + NG) * SWA + NGA + VX * lx;                       // in the halo tile
     constexpr int NE = 2 * NGV + VX;                                      // row values a thread reads
+    // Residual partials: one pair per (tile, chunk), flushed at every chunk boundary of the item and summed in
+    // a fixed order (thread: planes in order; then lanes, then warps), so the result does not depend on which
+    // CTA ran the chunk, when, or as part of how long an item (C16)
+    [[maybe_unused]] auto flush_partial = [&](int slot) {
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        num += __shfl_down_sync(0xffffffffu, num, o);
+        den += __shfl_down_sync(0xffffffffu, den, o);
+      }
+      if ((tid & 31) == 0) {
+        red[0][tid >> 5] = num;
+        red[1][tid >> 5] = den;
+      }
+      __syncthreads();
+      if (tid == 0) {
+        double sa = 0.0, sb = 0.0;
+#pragma unroll
+        for (int w = 0; w < NT / 32; ++w) {
+          sa += red[0][w];
+          sb += red[1][w];
+        }
+        ra.partials[2 * slot] = sa;
+        ra.partials[2 * slot + 1] = sb;
+      }
+      num = 0.0;
+      den = 0.0;
+    };
     int cz = col + z_begin * s2;  // stored index of this thread's first point in plane z
+    [[maybe_unused]] int zleft = plan.zc, pslot = tile_id * plan.nzc + ch0;  // planes left in the chunk, its partial slot
     for (int zb = z_begin; zb < z_end; zb += UR) {
 #pragma unroll
       for (int r = 0; r < UR; ++r) {
@@ -791,7 +835,7 @@ __global__ void __launch_bounds__((TW / VX) * BY,
             const F2 x = f2_add(L2(sb + ST_PSI * (TW * BY) + so), uc2);
             float x0, x1, r0, r1;
             f2_unpack(x, x0, x1);
-            bad |= !(x0 > 0.f) | (nact == VX & !(x1 > 0.f));
+            if constexpr (GUARD) bad |= !(x0 > 0.f) | (nact == VX & !(x1 > 0.f));
             asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r0) : "f"(x0));
             asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r1) : "f"(x1));
             F2 rr = f2_pack(r0, r1);
@@ -839,7 +883,7 @@ __global__ void __launch_bounds__((TW / VX) * BY,
                     z2v * d2;
             }
             const T x = psi.v[j] + HR_W(NG)[j];
-            bad |= j < nact & !(x > T(0));
+            if constexpr (GUARD) bad |= j < nact & !(x > T(0));
             H[j] = lap + Ss.v[j] * pow_m7(x);
           }
           }
@@ -963,6 +1007,12 @@ __global__ void __launch_bounds__((TW / VX) * BY,
           }
         }
         cz += s2;
+        if constexpr (RESID) {  // a chunk of the item is complete: its partial pair
+          if (--zleft == 0 || z + 1 == z_end) {
+            flush_partial(pslot++);
+            zleft = plan.zc;
+          }
+        }
 #undef HR_W
       }
       if constexpr (!HR_MARCH_ROTATE) {  // shift the window by the UR planes just done
@@ -973,32 +1023,6 @@ __global__ void __launch_bounds__((TW / VX) * BY,
       }
     }
     if (bad) *plan.flag = 1;
-    if constexpr (RESID) {
-      // one partial pair per ITEM, summed in a fixed order (thread: planes in order; then lanes,
-      // then warps), so the result does not depend on which CTA ran the item or when (C16)
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) {
-        num += __shfl_down_sync(0xffffffffu, num, o);
-        den += __shfl_down_sync(0xffffffffu, den, o);
-      }
-      if ((tid & 31) == 0) {
-        red[0][tid >> 5] = num;
-        red[1][tid >> 5] = den;
-      }
-      __syncthreads();
-      if (tid == 0) {
-        double sa = 0.0, sb = 0.0;
-#pragma unroll
-        for (int w = 0; w < NT / 32; ++w) {
-          sa += red[0][w];
-          sb += red[1][w];
-        }
-        ra.partials[2 * item] = sa;
-        ra.partials[2 * item + 1] = sb;
-      }
-      num = 0.0;
-      den = 0.0;
-    }
     if constexpr (ST == 5) {
       __syncthreads();  // red is reused by the next item
       item += gridDim.x;
@@ -1028,7 +1052,7 @@ __global__ void __launch_bounds__((TW / VX) * BY,
         // batches of 8 independent 16-byte loads, added in index order (latency-bound otherwise)
         const double2* pp = reinterpret_cast<const double2*>(ra.partials);
         int i = tid;
-        for (; i + 7 * NT < n_items; i += 8 * NT) {
+        for (; i + 7 * NT < n_part; i += 8 * NT) {
           double2 v[8];
 #pragma unroll
           for (int q = 0; q < 8; ++q) v[q] = __ldcg(pp + i + q * NT);
@@ -1038,7 +1062,7 @@ __global__ void __launch_bounds__((TW / VX) * BY,
             sb += v[q].y;
           }
         }
-        for (; i < n_items; i += NT) {
+        for (; i < n_part; i += NT) {
           const double2 v = __ldcg(pp + i);
           sa += v.x;
           sb += v.y;

@@ -478,19 +478,20 @@ def test_step_with_fused_residual(hr, name, params):
 
 
 def test_work_item_order_knobs_do_not_change_results(hr, monkeypatch):
-    """The (group, chunk, tile) decode of the marching kernels with ragged groups and chunks: tuning
-    knobs HR_TUNE_GT / HR_TUNE_ZC change the order in which work items run, never what they compute."""
-    params = W.sweep_point(7, (70, 99, 14), "SinhSymTP", 6)
+    """The work-item decode of the marching kernels (long items = segments of chunks, then single chunks, ragged
+    last chunk and last segment): tuning knobs HR_TUNE_COL / HR_TUNE_ZC change the order in which work runs and
+    how it is cut, never what is computed.  The grid has more tiles than CTA slots so that long items occur."""
+    params = W.sweep_point(7, (70, 1200, 14), "SinhSymTP", 6)
     o = Oracle(params)
     for dtype in ("f64", "f32"):
         u0, v0 = consistent_state(o, 21, dtype)
         ref = None
-        for gt, zc in ((None, None), ("7", "3"), ("10", "5"), ("1", "14")):
+        for gt, zc in ((None, None), ("7", "3"), ("10", "5"), ("1", "14"), ("0", "2")):
             if gt is None:
-                monkeypatch.delenv("HR_TUNE_GT", raising=False)
+                monkeypatch.delenv("HR_TUNE_COL", raising=False)
                 monkeypatch.delenv("HR_TUNE_ZC", raising=False)
-            else:
-                monkeypatch.setenv("HR_TUNE_GT", gt)
+            else:  # gt: here "long items on / off" (HR_TUNE_COL; 0 = single chunks only)
+                monkeypatch.setenv("HR_TUNE_COL", "0" if gt == "0" else "1")
                 monkeypatch.setenv("HR_TUNE_ZC", zc)
             s = hr.Solver(params, dtype=dtype)
             s.hr_set_state(u0, v0)
