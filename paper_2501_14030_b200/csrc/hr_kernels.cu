@@ -666,9 +666,22 @@ static void choose_chunks(MarchPlan& m, int n2, int ng, int slots, bool f64) {
     // fp64 with plenty of items (>= 4 rounds): 12 planes amortise the window priming better
     // (config 3: +1.5 %, 512x256x256: +3 %; on 128^3 8 planes stay ahead)
     if (f64 && ntiles * ((n2 + 11) / 12) >= 4LL * slots) zc = 12;
-    while (zc > 2 && ntiles * ((n2 + zc - 1) / zc) < slots) --zc;
-    // one plane per item where even that fits one wave of CTAs (config 0: the plane loop is a latency chain)
-    if (zc == 2 && ntiles * n2 <= slots) zc = 1;
+    if (ntiles * ((n2 + 7) / 8) < 4LL * slots) {
+      // Few waves of CTAs (L2-resident grids): a launch lasts waves x (planes per item + ~2 planes to prime the
+      // window and start the pipeline), each plane a ~1.2 us latency chain, so the item length is chosen to
+      // minimise that -- in particular never "just over one wave".  Ties go to the shorter item.  (Measured,
+      // config 2: fp64 4 planes 79.5 us per step against 84.6 at 8; config 0 / 1: 1 / 2 planes, one wave.)
+      long long best = -1;
+      for (int c = 1; c <= 16 && c <= n2; ++c) {
+        const int nz = (n2 + c - 1) / c, ce = (n2 + nz - 1) / nz;
+        const long long waves = (ntiles * nz + slots - 1) / slots;
+        const long long cost = waves * (ce + 2);
+        if (best < 0 || cost < best) {
+          best = cost;
+          zc = c;
+        }
+      }
+    }
   }
   if (zc > n2) zc = n2;
   m.nzc = (n2 + zc - 1) / zc;

@@ -540,16 +540,31 @@ __global__ void __launch_bounds__((TW / VX) * BY,
       } else {
         const int qo = m % g.n_o2;
         i2 = NG + m / g.n_o2;
-        const int po = a.OPOS[qo];
-        const int bits = po >> 28, q = po & 0x0fffffff;
-        i1 = q / g.T0;
-        i0 = q - i1 * g.T0;
-        c = g.off0 + i0 + g.P0 * i1 + s2 * i2;
         const T r0 = a.RAD0[qo], r1 = a.RAD1[qo], ri = a.RADI[qo];
-        uc = a.in_u[c];
-        vc = a.in_v[c];
-        ku = radiation_k(a.in_u, c, g.P0, r0, r1, ri, bits);
-        kv = radiation_k(a.in_v, c, g.P0, r0, r1, ri, bits);
+        if (plan.cyl) {  // C24: the list of outer positions of the plane with their stencil bits
+          const int po = a.OPOS[qo];
+          const int q = po & 0x0fffffff;
+          const int bits = po >> 28;
+          i1 = q / g.T0;
+          i0 = q - i1 * g.T0;
+          c = g.off0 + i0 + g.P0 * i1 + s2 * i2;
+          uc = a.in_u[c];
+          vc = a.in_v[c];
+          ku = radiation_k(a.in_u, c, g.P0, r0, r1, ri, bits);
+          kv = radiation_k(a.in_v, c, g.P0, r0, r1, ri, bits);
+        } else {
+          // spherical-like: the NG columns beyond x0 at interior rows, in list order; backward d_0, centred d_1
+          // (constant stencil bits: no dependent load and no branch between the loads -- on L2-resident grids
+          // this loop is on the critical path of the launch)
+          const int row = qo / NG;
+          i0 = g.n0 + NG + (qo - row * NG);
+          i1 = NG + row;
+          c = g.off0 + i0 + g.P0 * i1 + s2 * i2;
+          uc = a.in_u[c];
+          vc = a.in_v[c];
+          ku = radiation_k(a.in_u, c, g.P0, r0, r1, ri, 1);
+          kv = radiation_k(a.in_v, c, g.P0, r0, r1, ri, 1);
+        }
       }
       T wu, wv;
       if constexpr (LEAN) {
