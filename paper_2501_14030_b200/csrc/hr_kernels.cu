@@ -953,13 +953,17 @@ void hrk_replan(hr_solver* s, int share) {
   m.nseg = m.nzc;
   m.ncol = 0;
   const char* col_env = std::getenv("HR_TUNE_COL");  // tuning knob: 0 = chunks only
-  if (!(col_env && std::atoi(col_env) == 0) && ntiles * m.nzc >= 2LL * slots && m.nzc > 1) {
-    long long k = (slots + ntiles - 1) / ntiles;  // segments per tile: at least `slots` long items in all
-    if (k > m.nzc) k = m.nzc;
-    m.mseg = (int)((m.nzc + k - 1) / k);
-    m.nseg = (m.nzc + m.mseg - 1) / m.mseg;
-    m.ncol = (int)((ntiles * m.nseg / slots) * slots);
-    if (m.mseg == 1) m.ncol = 0;
+  // Long items = whole columns, for the first whole waves of CTAs, where a column is short enough for window
+  // priming to matter (<= 12 chunks) and there is at least one column per CTA; the remaining tiles' chunks are
+  // handed out one by one and absorb the CTAs whose tiles cost more (ghost images at the axis and the poles).
+  // Measured (burst, G point-substeps/s, columns / chunks only): config 3 fp64 73.9 / 70.2, 512x256x128 fp64 76.3 /
+  // 75.3, 512x256x256 fp64 85.9 / 87.0; segments shorter than a column, or columns on grids with fewer tiles than
+  // CTAs (every fp32 grid of the sweep: 256^3 fp32 100 against 130), never beat single chunks.
+  const bool want = col_env ? std::atoi(col_env) != 0 : true;
+  if (want && ntiles >= slots && m.nzc > 1 && m.nzc <= 12) {
+    m.mseg = m.nzc;
+    m.nseg = 1;
+    m.ncol = (int)((ntiles / slots) * slots);
   }
   const long long items = m.ncol + (ntiles * m.nseg - m.ncol) * m.mseg;
   for (int st = 0; st < 7; ++st) {
