@@ -124,6 +124,12 @@ struct HrArrays {
 #define HR_MARCH_UNROLL 2
 #endif
 
+// 1: the marching kernels are launched with programmatic stream serialization (PDL) and order themselves after
+// their predecessor with griddepcontrol.wait.
+#ifndef HR_MARCH_PDL
+#define HR_MARCH_PDL 1
+#endif
+
 // Planes of asynchronous look-ahead in the marching kernels.
 #ifndef HR_MARCH_D_F64
 #define HR_MARCH_D_F64 2

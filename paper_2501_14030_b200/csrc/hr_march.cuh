@@ -442,12 +442,20 @@ __global__ void __launch_bounds__((TW / VX) * BY,
   const int s2 = g.P0 * g.T1;
   const ImgGeom ig{NG, g.n2, g.T1, g.P0, g.off0, plan.sph};
 
+#if HR_MARCH_PDL
+  // PDL: let the next launch of the stream start its own set-up now ...
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+#endif
   if (tid == 0) {
 #pragma unroll
     for (int r = 0; r < RING; ++r) mbar_init(&bars[r], 1);
     mbar_fence_init();
   }
   __syncthreads();
+#if HR_MARCH_PDL
+  // ... and do not read or write anything the previous launch touches before it has completed
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+#endif
 
   // work items = (chunk of planes, tile), chunk-major
   const int ntiles = plan.ntx * plan.nty;
@@ -665,13 +673,6 @@ __global__ void __launch_bounds__((TW / VX) * BY,
         if (++sd == RING) sd = 0;
       }
     }
-    if constexpr (ADVANCE) {
-      if (!tail_done) {
-        outer_tail();
-        tail_done = true;
-      }
-    }
-
     // per-column constants
     T l00[VX], l11[VX], l22[VX], l0[VX], l1[VX], c2[VX];
     double wq[VX];
@@ -715,6 +716,15 @@ __global__ void __launch_bounds__((TW / VX) * BY,
 #pragma unroll
           for (int j = 0; j < VX; ++j) p[k][j] = t.v[j];
         }
+      }
+    }
+    // The outer-point loop runs once per CTA, here: after the first TMA copies, the per-column factors and the
+    // window priming loads have been ISSUED and before anything waits for them, so that its own load latency
+    // overlaps theirs (on L2-resident grids a CTA's life is one short item: serial latencies add up to the launch).
+    if constexpr (ADVANCE) {
+      if (!tail_done) {
+        outer_tail();
+        tail_done = true;
       }
     }
     [[maybe_unused]] F2 l00p{}, l11p{}, l22p{}, l0p{}, l1p{}, c2p{};
