@@ -670,11 +670,16 @@ static void choose_chunks(MarchPlan& m, int n2, int ng, int slots, bool f64) {
       // Few waves of CTAs (L2-resident grids): a launch lasts waves x (planes per item + ~2 planes to prime the
       // window and start the pipeline), each plane a ~1.2 us latency chain, so the item length is chosen to
       // minimise that -- in particular never "just over one wave".  Ties go to the shorter item.  (Measured,
-      // config 2: fp64 4 planes 79.5 us per step against 84.6 at 8; config 0 / 1: 1 / 2 planes, one wave.)
+      // config 2: fp64 4 planes 79.5 us per step against 84.6 at 8; config 0 / 1: 1 / 2 planes, one wave;
+      // the table of 16 grid / dtype cases x 7 lengths is in profiles/r2b.md.)
       long long best = -1;
       for (int c = 1; c <= 16 && c <= n2; ++c) {
         const int nz = (n2 + c - 1) / c, ce = (n2 + nz - 1) / nz;
         const long long waves = (ntiles * nz + slots - 1) / slots;
+        // one wave of LONG items leaves the SMs with 3-4 CTAs each running a long serial chain: measured 12-14 %
+        // behind two waves of shorter items (config 2 fp32: 7 planes 72.1 us against 3 planes 63.1; 256x128x64 fp32:
+        // 13 planes 108 us against 6 planes 93), so a single wave is only taken with items of <= 4 planes
+        if (waves == 1 && ce > 4) continue;
         const long long cost = waves * (ce + 2);
         if (best < 0 || cost < best) {
           best = cost;
