@@ -691,18 +691,7 @@ static void choose_chunks(MarchPlan& m, int n2, int ng, int slots, bool f64) {
   if (zc > n2) zc = n2;
   m.nzc = (n2 + zc - 1) / zc;
   m.zc = (n2 + m.nzc - 1) / m.nzc;
-  // Tiles per group: whole tile rows, about `gt_target` tiles.  Short chunks re-read the 2NG planes
-  // two consecutive chunks of a tile share; with all tiles in one group the second read comes a
-  // whole band of the grid later and misses L2.  Groups of ~256 tiles keep it in L2: fp64
-  // (DRAM-bound stages) +3 % on config 3; fp32 (issue-bound) -2 %, so fp32 keeps one group.
-  const char* gt_env = std::getenv("HR_TUNE_GT");  // tuning knob: tiles per group (0 = all)
-  const int gt_target = gt_env ? std::atoi(gt_env) : (f64 ? 256 : 0);
-  const int ntiles = m.ntx * m.nty;
-  int rows = gt_target > 0 ? (gt_target + m.ntx - 1) / m.ntx : m.nty;
-  if (rows < 1) rows = 1;
-  if (rows > m.nty) rows = m.nty;
-  m.gt = rows * m.ntx;
-  (void)ntiles;
+  m.gt = m.ntx * m.nty;  // (round 1's groups of tile rows are gone: long items took over their job)
 }
 
 // Persistent grid of one stage's kernel: resident CTAs per SM x SMs (never more than the work).

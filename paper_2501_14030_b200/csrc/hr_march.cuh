@@ -14,20 +14,24 @@
 //     that copy of the loop no longer fits the 32 KB instruction cache and measured no faster);
 //   * fp32: a thread owns two points and does the i1 / i2 stencils, the metric combination, the
 //     source term and the RK combine on packed pairs (fma/add/mul.f32x2 -> FFMA2 / FADD2 / FMUL2);
-//   * CTAs are persistent over (chunk of planes, tile) work items, chunk-major within groups of
-//     tile rows, so the CTAs resident at any time work on neighbouring tiles of the same planes
-//     (halo rows meet in L2) and the chunks of a tile follow each other while the planes their
-//     windows share are still in L2; after its first item a CTA takes the next one from an
-//     atomic counter;
+//   * CTAs are persistent over work items: whole columns of a tile for the first whole waves of
+//     CTAs where a column is short (config 3), then (chunk of planes, tile) items, chunk-major, so the
+//     CTAs resident at any time work on neighbouring tiles of the same planes (halo rows meet in
+//     L2); after its first item a CTA takes the next one from an atomic counter, unless there are
+//     no more items than CTAs;
 //   * the reference-metric factors depend on (i0, i1) only (reading C4), so each thread loads its
 //     six coefficients once per column and keeps them in registers;
 //   * the RK combine (a4) happens in the same thread, so k never reaches HBM (default: classic RK4
 //     without a running sum, STAGE codes 11-14 and 16, 32w bytes per point and step; STAGE 1-4
-//     and 6: the running-sum form, variant 3, 40w), and the thread that
+//     and 6: the running-sum form, variant 3, 40w; fp32 takes the increment-preserving stages 22 / 24,
+//     34w), and the thread that
 //     produces a point also writes that point's inner-ghost images (a3, reading C14/C15) --
 //     closed-form integer arithmetic, the inverse of the host's inner map -- so a substep is
 //     one launch;
-//   * the outer (radiation) points are a grid-stride loop at the end of the same kernel.
+//   * the outer (radiation) points are a grid-stride loop of the same kernel, run by every CTA once
+//     the first loads of its first item are in flight; CART = the SinhCartesian instantiation (C25);
+//   * launched with programmatic stream serialization: launch_dependents at entry,
+//     griddepcontrol.wait before the first access to what the previous substep wrote.
 // Included by hr_kernels.cu only.
 #pragma once
 
