@@ -538,3 +538,31 @@ def test_poisoned_workspace_changes_nothing(hr, name, params):
             s.close()
         for a, b in zip(*got):
             assert np.array_equal(a, b) and np.isfinite(a).all()
+
+
+def test_query_and_measurement_hooks(hr):
+    """hr_query (which path runs, the plan, the numeric flag) and the two measurement hooks of include/hr.h."""
+    s = hr.Solver(W.config(1))
+    assert s.hr_query("step_graph") == 1          # hr_step replays the captured graph, not the fallback
+    assert s.hr_query("persistent") == 0
+    assert s.hr_query("numeric_flag") == 0
+    zc, items, grid = s.hr_query("plan_zc"), s.hr_query("plan_items"), s.hr_query("plan_grid")
+    assert 1 <= zc <= 16 and items >= 64 and 1 <= grid <= items
+    import torch
+    out2 = torch.zeros(2, dtype=torch.float64, device=s.device)
+    s.hr_step_residual_async(0, out2)
+    s.synchronize()
+    assert s.hr_query("resid_graph") & 1
+    # a state that drives psi_BL + u through zero is reported, and a new state clears the flag
+    bad = np.full(s.ntot, -5.0)
+    s.hr_set_state(bad, np.zeros(s.ntot))
+    with pytest.raises(hr.HrError) as e:
+        s.hr_residual(0)
+    assert e.value.status == 5 and s.hr_query("numeric_flag") != 0
+    s.hr_set_state(np.zeros(s.ntot), np.zeros(s.ntot))
+    assert s.hr_query("numeric_flag") == 0 and s.hr_residual(0) > 0
+    s.close()
+    f64, f32 = hr.hr_measure_alu_peak("f64"), hr.hr_measure_alu_peak("f32", packed=True)
+    assert 15.0 < f64 < 60.0 and 40.0 < f32 < 120.0 and f32 > 1.5 * f64, (f64, f32)  # TFLOP/s on a B200
+    floor = hr.hr_measure_launch_floor(4, 148, 128, 200)
+    assert 1.0 < floor < 50.0, floor  # microseconds per replay of a 4-launch graph
