@@ -126,9 +126,45 @@ def run_sweep():
     np.savez_compressed(os.path.join(HERE, "full_config4.npz"), **arrays)
 
 
+# f3 (readings C24 / C25): the cylindrical-like and Cartesian-like systems at sweep sizes, same recipe
+F3_GRIDS = [(128, 128, 128), (256, 128, 64)]
+
+
+def f3_cases():
+    k = 200
+    for n in F3_GRIDS:
+        for coord in ("SinhCylindrical", "SinhCartesian"):
+            for order in SWEEP_ORDERS:
+                yield k, n, coord, order
+                k += 1
+
+
+def run_f3():
+    arrays = {}
+    t0 = time.time()
+    for k, n, coord, order in f3_cases():
+        p = W.sweep_point(k, n, coord, order)
+        o = Oracle(p)
+        idx = sample_indices(o, SAMPLE_SEED + k, 4096, 2048, 1024) if o.n_inner > 0 else np.sort(
+            np.random.default_rng(SAMPLE_SEED + k).choice(o.ntot, size=8192, replace=False)).astype(np.int64)
+        u, v = W.random_state(o.ntot, seed=1000 + k)
+        u, v = o.apply_inner(u), o.apply_inner(v)
+        ku, kv = o.rhs(u, v)
+        u32, v32 = u.astype(np.float32), v.astype(np.float32)
+        ku32, kv32 = o.rhs(u32.astype(np.float64), v32.astype(np.float64))
+        arrays[f"idx_{k}"] = idx
+        arrays[f"ku_{k}"], arrays[f"kv_{k}"] = ku[idx], kv[idx]
+        arrays[f"ku32in_{k}"], arrays[f"kv32in_{k}"] = ku32[idx], kv32[idx]
+        arrays[f"kmax_{k}"] = np.array([np.abs(ku).max(), np.abs(kv).max(), np.abs(ku32).max(), np.abs(kv32).max()])
+        print("f3", k, n, coord, order, "%.0f s" % (time.time() - t0), flush=True)
+    np.savez_compressed(os.path.join(HERE, "full_f3.npz"), **arrays)
+
+
 if __name__ == "__main__":
     for name in sys.argv[1:]:
         if name == "config4":
             run_sweep()
+        elif name == "f3":
+            run_f3()
         else:
             run_case(name)

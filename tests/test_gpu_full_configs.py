@@ -199,3 +199,43 @@ def test_sweep_grids_full_size_rhs(hr, dtype):
         s.close()
         del ku, kv, u, v
     emit("config4", dtype, lines)
+
+
+def f3_cases():
+    k = 200
+    for n in [(128, 128, 128), (256, 128, 64)]:
+        for coord in ("SinhCylindrical", "SinhCartesian"):
+            for order in (4, 10):
+                yield k, n, coord, order
+                k += 1
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_f3_reference_metrics_at_sweep_sizes(hr, dtype):
+    """The cylindrical-like and Cartesian-like systems (readings C24 / C25) at two sweep sizes, orders 4 and 10: one
+    RHS evaluation against the oracle's k on 8192 sampled points each (interior, the outer points of every face,
+    inner ghosts where the system has them); same bars as configs[4]."""
+    path = os.path.join(GOLD, "full_f3.npz")
+    if not os.path.exists(path):
+        pytest.skip("full_f3.npz not written yet (python tests/golden/make_golden_full.py f3)")
+    z = np.load(path)
+    tol = 1e-12 if dtype == "f64" else 1e-5
+    lines = [f"# f3 grids {dtype}: per-RHS max-norm relative error on the sampled points (bar {tol:g})",
+             "# k grid coord order err_ku err_kv"]
+    for k, n, coord, order in f3_cases():
+        p = W.sweep_point(k, n, coord, order)
+        s = hr.Solver(p, dtype=dtype)
+        u, v = W.random_state(s.ntot, seed=1000 + k)
+        if dtype == "f32":
+            u, v = u.astype(np.float32), v.astype(np.float32)
+        s.hr_set_state(u, v)
+        ku, kv = s.hr_eval_rhs()
+        idx = z[f"idx_{k}"]
+        tag = "32in" if dtype == "f32" else ""
+        kmax = z[f"kmax_{k}"][2:] if dtype == "f32" else z[f"kmax_{k}"][:2]
+        eu = np.abs(ku[idx].astype(np.float64) - z[f"ku{tag}_{k}"]).max() / kmax[0]
+        ev = np.abs(kv[idx].astype(np.float64) - z[f"kv{tag}_{k}"]).max() / kmax[1]
+        lines.append(f"{k} {n[0]}x{n[1]}x{n[2]} {coord} {order} {eu:.2e} {ev:.2e}")
+        assert eu <= tol and ev <= tol, (k, n, coord, order, eu, ev)
+        s.close()
+    emit("f3", dtype, lines)
