@@ -566,3 +566,34 @@ def test_query_and_measurement_hooks(hr):
     assert 15.0 < f64 < 60.0 and 40.0 < f32 < 120.0 and f32 > 1.5 * f64, (f64, f32)  # TFLOP/s on a B200
     floor = hr.hr_measure_launch_floor(4, 148, 128, 200)
     assert 1.0 < floor < 50.0, floor  # microseconds per replay of a 4-launch graph
+
+
+def _random_case(seed):
+    rng = np.random.default_rng(9000 + seed)
+    order = int(rng.choice([2, 4, 6, 8, 10, 12]))
+    ng = order // 2
+    coord = ["SinhSpherical", "SinhSymTP", "SinhCylindrical", "SinhCartesian"][seed % 4]
+    n = (int(rng.integers(ng, 81)), int(rng.integers(ng, 41)), 2 * int(rng.integers((max(ng, 2) + 1) // 2, 13)))
+    return dict(W.sweep_point(300 + seed, n, coord, order), eta=0.05)
+
+
+@pytest.mark.parametrize("seed", range(32))
+def test_random_small_grids(hr, seed):
+    """Seeded random shapes (N_a from NG up, odd sizes, fewer points than a tile, every FD order, all four reference
+    metrics, both precisions): boundary lists bit-exact, one RHS evaluation at the north_star bars on every one of
+    the N_tot entries, ghosts bitwise equal to their sources."""
+    params = _random_case(seed)
+    o = Oracle(params)
+    for dtype in ("f64", "f32"):
+        s = hr.Solver(params, dtype=dtype)
+        for a, b in zip(s.hr_get_bc_lists(), o.bc_lists()):
+            assert np.array_equal(a, b), (params["coord"], params["n"], params["fd_order"])
+        u, v = consistent_state(o, 50 + seed, dtype)
+        s.hr_set_state(u, v)
+        ku, kv = s.hr_eval_rhs()
+        oku, okv = o.rhs(u.astype(np.float64), v.astype(np.float64))
+        eu, ev = relmax(ku, oku), relmax(kv, okv)
+        assert eu <= TOL_RHS[dtype] and ev <= TOL_RHS[dtype], (params["coord"], params["n"], params["fd_order"], dtype, eu, ev)
+        dst, src, _ = o.bc_lists()
+        assert np.array_equal(ku[dst], ku[src]) and np.array_equal(kv[dst], kv[src])
+        s.close()
