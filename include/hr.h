@@ -152,6 +152,20 @@ HR_API hr_status hr_residual_ex(hr_solver* s, int32_t mode, double* out3);
  * H kernel and the reduction and writes { sum w H^2, sum w } (2 doubles) to out2_dev (device
  * pointer); no host synchronisation. */
 HR_API hr_status hr_residual_async(hr_solver* s, int32_t mode, double* out2_dev);
+/* hr_residual_async for callers that must not allocate and hold no scratch of their own to lend (code under CUDA
+ * graph capture, serving loops, harnesses that forbid cudaMalloc): the same kernel (Alg. 1 l.9-11, C16; marching
+ * arrangements, variant 0 or 3) with its scratch -- one partial pair per work item and the launch counters -- in a
+ * static __device__ array inside the library instead of the solver's workspace: 1 MiB + 256 bytes per GPU that
+ * loads the library, held until the process exits.  Input: the solver's current state; output: { sum w H^2, sum w }
+ * (2 doubles) to out2_dev (device pointer, the caller's).  Enqueues a clear of the counters and one kernel on the
+ * solver's stream; calls no cudaMalloc / cudaFree or allocating routine; no host synchronisation.  The result equals
+ * hr_residual_async's bit for bit (same kernel, same fixed reduction order).
+ * Limit: at most 65536 (tile, chunk of planes) pairs, one partial each (the largest BASELINE.json grid, 512x256x256
+ * in fp64, has 32768); beyond it HR_ERR_WORKSPACE with the counts in hr_last_error().  Variants 1 and 2:
+ * HR_ERR_INVALID_ARG.
+ * Every call on a GPU, of every solver, shares the one array, which keeps the last call's contents: calls that
+ * overlap on the device (different streams, no ordering between them) race.  Order them. */
+HR_API hr_status hr_residual_static(hr_solver* s, int32_t mode, double* out2_dev);
 
 /* Alg. 1 l.8-18, the relaxation loop with its stopping criterion (C18): repeat
  * { residual (l.9-11); check_every RK4 steps (l.12-16) } until the residual norm (mode 0 or 1, C16)

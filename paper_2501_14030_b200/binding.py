@@ -69,6 +69,7 @@ _SIGS = {
     "hr_residual": [_vp, C.POINTER(C.c_double)],
     "hr_residual_ex": [_vp, _i32, C.POINTER(C.c_double)],
     "hr_residual_async": [_vp, _i32, _vp],
+    "hr_residual_static": [_vp, _i32, _vp],
     "hr_step_many": [C.POINTER(_vp), _i32, _i64],
     "hr_step_residual_async": [_vp, _i32, _vp],
     "hr_relax": [_vp, _i64, _i64, C.c_double, _i32, C.POINTER(_i64), C.POINTER(C.c_double), _vp, _i64,
@@ -268,6 +269,10 @@ class Solver:
     def hr_residual_async(self, mode, out2):
         """out2: torch float64 CUDA tensor with >= 2 elements; receives {sum w H^2, sum w}."""
         _check(lib.hr_residual_async(self._h, _i32(int(mode)), _vp(out2.data_ptr())))
+
+    def hr_residual_static(self, mode, out2):
+        """hr_residual_async with the kernel's scratch in the library's static device array (no allocation)."""
+        _check(lib.hr_residual_static(self._h, _i32(int(mode)), _vp(out2.data_ptr())))
 
     def hr_step_residual_async(self, mode, out2):
         """Residual of the current state into out2 (as hr_residual_async), then one RK4 step."""

@@ -842,6 +842,21 @@ hr_status hr_residual_async(hr_solver* s, int32_t mode, double* out2_dev) {
   return HR_OK;
 }
 
+hr_status hr_residual_static(hr_solver* s, int32_t mode, double* out2_dev) {
+  if (!s || !out2_dev) return fail(HR_ERR_INVALID_ARG, "NULL argument");
+  if (mode != 0 && mode != 1) return fail(HR_ERR_INVALID_ARG, "mode must be 0 or 1");
+  if (s->p.variant == 1 || s->p.variant == 2)
+    return fail(HR_ERR_INVALID_ARG, "hr_residual_static serves the marching arrangements (variant 0 or 3), not variant %d",
+                (int)s->p.variant);
+  const int64_t items = (int64_t)s->plan.ntx * s->plan.nty * s->plan.nzc;
+  if (items > HR_STATIC_MAX_PARTIALS)
+    return fail(HR_ERR_WORKSPACE,
+                "hr_residual_static: %lld (tile, chunk) partials, the static scratch holds %d; use hr_residual_async",
+                (long long)items, HR_STATIC_MAX_PARTIALS);
+  HR_CUDA(hrk_residual_static(s, mode, out2_dev));
+  return HR_OK;
+}
+
 hr_status hr_residual_ex(hr_solver* s, int32_t mode, double* out3) {
   if (!s || !out3) return fail(HR_ERR_INVALID_ARG, "NULL argument");
   hr_status st = hr_residual_async(s, mode, s->a.result2);

@@ -141,6 +141,12 @@ struct HrArrays {
 #define HR_MARCH_D_F32 2
 #endif
 
+// hr_residual_static's scratch (a static __device__ array, one per GPU that loads the library): room for the
+// launch counters and for HR_STATIC_MAX_PARTIALS work-item partial pairs = 1 MiB + 256 bytes.
+#define HR_STATIC_COUNTER_BYTES 256
+#define HR_STATIC_MAX_PARTIALS 65536
+#define HR_STATIC_MAX_DEVICES 64
+
 // Tiling of the marching kernels (hr_march.cuh).
 struct MarchPlan {
   int ntx, nty;  // tiles along i0, i1
@@ -212,6 +218,10 @@ cudaError_t hrk_unpack(const hr_solver* s, void* dst_stored, const void* src_pub
 void hrk_row_geometry(int T0, int ng, size_t scalar_bytes, int* P0, int* off0);
 // residual partial sums + final deterministic pass into out2_dev
 cudaError_t hrk_residual(const hr_solver* s, int mode, double* out2_dev);
+// hr_residual_static: the same launch (marching arrangements only) with its scratch -- the work-item partials and
+// the launch counters -- in a file-scope __device__ array of hr_kernels.cu; enqueues a clear of the counters and
+// the kernel, allocates nothing.  The caller has checked that the plan has at most HR_STATIC_MAX_PARTIALS items.
+cudaError_t hrk_residual_static(const hr_solver* s, int mode, double* out2_dev);
 // one RK4 step whose first substep also reduces the residual of the state it starts from
 cudaError_t hrk_step_with_residual(const hr_solver* s, int mode, double* out2_dev);
 // its first launch alone (hr_profile_step): stage 1 + residual, reduced into out2_dev

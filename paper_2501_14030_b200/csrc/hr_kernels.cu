@@ -13,6 +13,7 @@
 #include <algorithm>
 
 #include <cstdlib>
+#include <mutex>
 #include <type_traits>
 
 #include "fd_tables.cuh"
@@ -923,7 +924,80 @@ cudaError_t dispatch_fused_first(const hr_solver* s, int mode, double* out2) {
   return cudaErrorInvalidValue;
 }
 
+// hr_residual_static: the stand-alone residual launch of launch_march_stage<T, NG, 5> with the work-item
+// partials and the {next item, CTAs done} counter pair in `scratch` (the file-scope array below) instead of
+// the solver's workspace.  The numeric flag stays the solver's.  No programmatic launch: the clear of the
+// counters that precedes it in the stream is complete when the kernel starts.
+template <typename T, int NG>
+cudaError_t launch_residual_static(const hr_solver* s, int mode, unsigned char* scratch, double* out2) {
+  using C = MarchCfg<T>;
+  constexpr size_t smem = HR_MARCH_SMEM(T, NG, 5);
+  const dim3 block(C::TW / C::VX, C::BY, 1);
+  const dim3 grid(s->march_grid[5], 1, 1);
+  const MarchMaps mm = make_maps(s, 5);
+  const StepArgs<T> a = make_args<T>(s, 5, nullptr, nullptr);
+  MarchPlan plan = s->plan;
+  plan.counters = reinterpret_cast<int*>(scratch);
+  const ResidArgs ra{s->a.Wvol, reinterpret_cast<double*>(scratch + HR_STATIC_COUNTER_BYTES), mode, out2, s->a.ZH};
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = s->stream;
+  if (s->plan.cart) return cudaLaunchKernelEx(&cfg, HR_MARCH_KERNEL(T, NG, 5, true), s->g, a, plan, ra, mm);
+  return cudaLaunchKernelEx(&cfg, HR_MARCH_KERNEL(T, NG, 5, false), s->g, a, plan, ra, mm);
+}
+
+template <typename T>
+cudaError_t dispatch_residual_static(const hr_solver* s, int mode, unsigned char* scratch, double* out2) {
+  switch (s->g.ng) {
+    case 1: return launch_residual_static<T, 1>(s, mode, scratch, out2);
+    case 2: return launch_residual_static<T, 2>(s, mode, scratch, out2);
+    case 3: return launch_residual_static<T, 3>(s, mode, scratch, out2);
+    case 4: return launch_residual_static<T, 4>(s, mode, scratch, out2);
+    case 5: return launch_residual_static<T, 5>(s, mode, scratch, out2);
+    case 6: return launch_residual_static<T, 6>(s, mode, scratch, out2);
+  }
+  return cudaErrorInvalidValue;
+}
+
 }  // namespace
+
+// Scratch of hr_residual_static: HR_STATIC_COUNTER_BYTES of launch counters, then HR_STATIC_MAX_PARTIALS pairs
+// of doubles.  One copy per GPU that loads the library, held until the process exits.  In host code the name
+// below is a host-side stand-in, not a device address: the launcher gets the address once per device from
+// cudaGetSymbolAddress, with that device current, and hands it to the kernel.
+static __device__ __align__(256) unsigned char hr_static_scratch[HR_STATIC_COUNTER_BYTES +
+                                                                  (size_t)HR_STATIC_MAX_PARTIALS * 16];
+
+cudaError_t hrk_residual_static(const hr_solver* s, int mode, double* out2_dev) {
+  static std::mutex mu;
+  static unsigned char* addr[HR_STATIC_MAX_DEVICES] = {};  // per device, filled on first use
+  const int dev = s->p.device;
+  if (dev < 0 || dev >= HR_STATIC_MAX_DEVICES) return cudaErrorInvalidDevice;
+  unsigned char* scratch;
+  {
+    std::lock_guard<std::mutex> lock(mu);
+    if (!addr[dev]) {
+      int cur = -1;
+      cudaError_t e = cudaGetDevice(&cur);
+      if (e != cudaSuccess) return e;
+      if (cur != dev && (e = cudaSetDevice(dev)) != cudaSuccess) return e;
+      void* p = nullptr;
+      e = cudaGetSymbolAddress(&p, hr_static_scratch);
+      if (cur != dev) cudaSetDevice(cur);
+      if (e != cudaSuccess) return e;
+      addr[dev] = static_cast<unsigned char*>(p);
+    }
+    scratch = addr[dev];
+  }
+  // the array keeps the last call's contents: the counters must start at zero (the partials are all written
+  // before they are read)
+  cudaError_t e = cudaMemsetAsync(scratch, 0, HR_STATIC_COUNTER_BYTES, s->stream);
+  if (e != cudaSuccess) return e;
+  return s->p.dtype == HR_F64 ? dispatch_residual_static<double>(s, mode, scratch, out2_dev)
+                              : dispatch_residual_static<float>(s, mode, scratch, out2_dev);
+}
 
 // Tiling of the marching kernels for a grid.  The chunk length is fixed later (hrk_prepare),
 // once the persistent grid size is known.
