@@ -162,6 +162,13 @@ struct alignas(64) MarchMaps {
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
   return (uint32_t)__cvta_generic_to_shared(p);
 }
+// one lane of a converged warp (the TMA issue then compiles to straight-line uniform-datapath code instead of a
+// loop over the active lanes of a divergent branch)
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile("{\n.reg .pred P;\nelect.sync _|P, 0xffffffff;\nselp.u32 %0, 1, 0, P;\n}\n" : "=r"(pred));
+  return pred != 0;
+}
 __device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count) : "memory");
 }
@@ -184,8 +191,19 @@ __device__ __forceinline__ unsigned long long global_timer_ns() {
   asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
   return t;
 }
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t phase) {
+__device__ __forceinline__ uint32_t mbar_try_wait(uint32_t bar, uint32_t phase) {
   uint32_t ok;
+  asm volatile(
+      "{\n.reg .pred p;\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+      "selp.u32 %0, 1, 0, p;\n}\n"
+      : "=r"(ok)
+      : "r"(bar), "r"(phase)
+      : "memory");
+  return ok;
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t phase) {
+  if (mbar_try_wait(bar, phase)) return;  // the common case costs one instruction and a branch
   [[maybe_unused]] uint32_t spins = 0;
   [[maybe_unused]] unsigned long long t0 = 0;
   do {
@@ -196,14 +214,7 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t phase) {
       else if (now - t0 > HR_MBAR_TIMEOUT_NS) __trap();
     }
 #endif
-    asm volatile(
-        "{\n.reg .pred p;\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
-        "selp.u32 %0, 1, 0, p;\n}\n"
-        : "=r"(ok)
-        : "r"(bar), "r"(phase)
-        : "memory");
-  } while (!ok);
+  } while (!mbar_try_wait(bar, phase));
 }
 // L2 eviction policies for the loads: the pointwise inputs are read once per substep
 // (evict first), u is read again by the neighbouring tiles and, NG planes later, as a halo tile
@@ -442,6 +453,7 @@ __global__ void __launch_bounds__((TW / VX) * BY,
 
   const int lx = threadIdx.x, ly = threadIdx.y;
   const int tid = ly * BXT + lx;
+  const bool warp0 = __shfl_sync(0xffffffffu, tid >> 5, 0) == 0;  // warp-uniform, and known to be
   constexpr bool is_cart = CART;  // SinhCartesian (C25)
   const int s2 = g.P0 * g.T1;
   const ImgGeom ig{NG, g.n2, g.T1, g.P0, g.off0, plan.sph};
@@ -669,7 +681,7 @@ __global__ void __launch_bounds__((TW / VX) * BY,
       for (int q = 1; q < NS; ++q) tma_load_3d(sb + q * G::BOX_BYTES, &mm.st[q], xs, y0, zz, bar);
 #endif
     };
-    if (tid == 0) {
+    if (warp0 && elect_one()) {
       int sd = sl;
 #pragma unroll
       for (int d = 0; d < D; ++d) {
@@ -780,7 +792,9 @@ __global__ void __launch_bounds__((TW / VX) * BY,
         if (z >= z_end) break;
 #define HR_W(k) p[HR_MARCH_ROTATE ? (r + (k)) % U : r + (k)]
         __syncthreads();  // every thread is done with plane z-1: its slot can be refilled
-        if (tid == 0 && z + D < z_end) issue(z + D, sl == 0 ? RING - 1 : sl - 1);  // (sl + D) % RING
+        if (warp0 && z + D < z_end) {
+          if (elect_one()) issue(z + D, sl == 0 ? RING - 1 : sl - 1);  // (sl + D) % RING
+        }
         mbar_wait(bars_u32 + sl * 8, par);  // the boxes of plane z have landed
         const T* tl = reinterpret_cast<const T*>(ring + sl * SLOT_BYTES);
         const T* sb = reinterpret_cast<const T*>(ring + sl * SLOT_BYTES + G::TILE_BYTES);
