@@ -30,8 +30,9 @@
 //     one launch;
 //   * the outer (radiation) points are a grid-stride loop of the same kernel, run by every CTA once
 //     the first loads of its first item are in flight; CART = the SinhCartesian instantiation (C25);
-//   * launched with programmatic stream serialization: launch_dependents at entry,
-//     griddepcontrol.wait before the first access to what the previous substep wrote.
+//   * launched with programmatic stream serialization: launch_dependents at entry where every CTA has one
+//     item (small grids), after the item loop where items are handed out; griddepcontrol.wait before the
+//     first access to what the previous substep wrote.
 // Included by hr_kernels.cu only.
 #pragma once
 
@@ -458,9 +459,20 @@ __global__ void __launch_bounds__((TW / VX) * BY,
   const int s2 = g.P0 * g.T1;
   const ImgGeom ig{NG, g.n2, g.T1, g.P0, g.off0, plan.sph};
 
+  // work items = (chunk of planes, tile), chunk-major
+  const int ntiles = plan.ntx * plan.nty;
+  const int n_long = ntiles * plan.nseg;                              // segments of plan.mseg chunks
+  const int n_items = plan.ncol + (n_long - plan.ncol) * plan.mseg;   // long items, then single chunks
+  const int n_part = ntiles * plan.nzc;                               // residual partials: one per (tile, chunk)
+  // no more items than CTAs (small grids): every CTA has exactly one item, nothing is handed out, and
+  // no atomic round trip sits at the end of the CTA's (short) life
+  const bool dynamic = n_items > (int)gridDim.x;
 #if HR_MARCH_PDL
-  // PDL: let the next launch of the stream start its own set-up now ...
-  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  // PDL: let the next launch of the stream start its own set-up now ... -- on small grids only, where a CTA
+  // lives for one short item and the next launch's start-up is worth hiding.  Where items are handed out, the
+  // CTAs of the next launch would sit in the slots of those that are done while the last ones still march:
+  // measured up to 30 % slower per step (profiles/r2c.md), so there the trigger is left to the end of the grid.
+  if (!dynamic) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 #endif
   if (tid == 0) {
 #pragma unroll
@@ -473,14 +485,6 @@ __global__ void __launch_bounds__((TW / VX) * BY,
   asm volatile("griddepcontrol.wait;" ::: "memory");
 #endif
 
-  // work items = (chunk of planes, tile), chunk-major
-  const int ntiles = plan.ntx * plan.nty;
-  const int n_long = ntiles * plan.nseg;                              // segments of plan.mseg chunks
-  const int n_items = plan.ncol + (n_long - plan.ncol) * plan.mseg;   // long items, then single chunks
-  const int n_part = ntiles * plan.nzc;                               // residual partials: one per (tile, chunk)
-  // no more items than CTAs (small grids): every CTA has exactly one item, nothing is handed out, and
-  // no atomic round trip sits at the end of the CTA's (short) life
-  const bool dynamic = n_items > (int)gridDim.x;
 
   double num = 0.0, den = 0.0;
   bool bad = false;  // psi_BL + u <= 0 or NaN met at an interior point (the device flag)
@@ -1077,6 +1081,10 @@ __global__ void __launch_bounds__((TW / VX) * BY,
       item = s_item;
     }
   }
+#if HR_MARCH_PDL
+  // (dynamic hand-out) this CTA marches no more: once all have said so the next launch may move in
+  if (dynamic) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+#endif
   // The last CTA to leave the item loop re-arms the counters for the next launch of this stage
   // and, for the residual stages, sums the item partials in a fixed order (thread t takes items
   // t, t + NT, ...; then a fixed tree), so the reduction needs no launch of its own and its
