@@ -162,6 +162,8 @@ struct MarchPlan {
   int cart;      // 1 = SinhCartesian (C25): u_2 term, x2-dependent factors, six outer faces, no images
   int cyl;       // 1 = SinhCylindrical (C24): x1 is axial, no theta reflections, outer points beyond its ends
   int* flag;     // device: set non-zero by a kernel that meets psi_BL + u <= 0 or NaN at an interior point
+  int pdl;       // programmatic-launch trigger: 1 = at entry where every CTA has one item, 0 = always after the
+                 // item loop (solvers that share the GPU in hr_step_many), 2 = always at entry (HR_TUNE_PDL)
 };
 
 struct hr_solver {

@@ -1031,6 +1031,9 @@ void hrk_replan(hr_solver* s, int share) {
   m.mseg = 1;
   m.nseg = m.nzc;
   m.ncol = 0;
+  // CTAs of the next launch that move in early wait in slots that the kernels of the other solvers could run in
+  const char* pdl_env = std::getenv("HR_TUNE_PDL");  // tuning knob: 0 / 1 / 2, see MarchPlan::pdl
+  m.pdl = pdl_env ? std::atoi(pdl_env) : (share == 1 ? 1 : 0);
   const char* col_env = std::getenv("HR_TUNE_COL");  // tuning knob: 0 = chunks only
   // Long items = whole columns, for the first whole waves of CTAs, where a column is short enough for window
   // priming to matter (<= 12 chunks) and there is at least one column per CTA; the remaining tiles' chunks are

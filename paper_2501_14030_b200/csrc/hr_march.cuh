@@ -472,7 +472,8 @@ __global__ void __launch_bounds__((TW / VX) * BY,
   // lives for one short item and the next launch's start-up is worth hiding.  Where items are handed out, the
   // CTAs of the next launch would sit in the slots of those that are done while the last ones still march:
   // measured up to 30 % slower per step (profiles/r2c.md), so there the trigger is left to the end of the grid.
-  if (!dynamic) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  const bool pdl_early = plan.pdl == 2 || (plan.pdl == 1 && !dynamic);
+  if (pdl_early) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 #endif
   if (tid == 0) {
 #pragma unroll
@@ -1082,8 +1083,8 @@ __global__ void __launch_bounds__((TW / VX) * BY,
     }
   }
 #if HR_MARCH_PDL
-  // (dynamic hand-out) this CTA marches no more: once all have said so the next launch may move in
-  if (dynamic) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  // (dynamic hand-out, shared GPU) this CTA marches no more: once all have said so the next launch may move in
+  if (!pdl_early) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 #endif
   // The last CTA to leave the item loop re-arms the counters for the next launch of this stage
   // and, for the residual stages, sums the item partials in a fixed order (thread t takes items
