@@ -1,5 +1,8 @@
 """The oracle reproduces its committed regression anchors (tests/golden/oracle_residuals.txt,
-written by tests/golden/make_golden.py from oracle/ only)."""
+written by tests/golden/make_golden.py from oracle/ only).
+
+This compares the oracle with its own earlier output: it guards against an unnoticed change of the oracle's
+arithmetic between commits, and pins nothing.  What pins the oracle is in tests/test_oracle_pins*.py."""
 import os
 
 import pytest
