@@ -162,6 +162,9 @@ struct MarchPlan {
   int cart;      // 1 = SinhCartesian (C25): u_2 term, x2-dependent factors, six outer faces, no images
   int cyl;       // 1 = SinhCylindrical (C24): x1 is axial, no theta reflections, outer points beyond its ends
   int* flag;     // device: set non-zero by a kernel that meets psi_BL + u <= 0 or NaN at an interior point
+  // quotients of the work-item decode by multiplication: q = umulhi(n, mul) >> shr for 0 <= n < 2^31 (mul = 0: the
+  // divisor is 1 or unused), for the divisors ntx * nty, ntx and ntx * nty * nseg - ncol; set by hrk_replan
+  uint32_t dv_tiles[2], dv_ntx[2], dv_rem[2];
   int pdl;       // programmatic-launch trigger: 1 = at entry where every CTA has one item, 0 = always after the
                  // item loop (solvers that share the GPU in hr_step_many), 2 = always at entry (HR_TUNE_PDL)
 };

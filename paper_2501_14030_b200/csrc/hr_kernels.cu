@@ -1020,6 +1020,20 @@ MarchPlan hrk_make_plan(const int32_t n[3], int ng, int coord, int dtype) {
   return m;
 }
 
+// Division of 0 <= n < 2^31 by a launch-invariant d >= 1 as a multiplication (Granlund & Montgomery 1994):
+// p = 31 + ceil(log2 d), mul = ceil(2^p / d), n / d = umulhi(n, mul) >> (p - 32).  The item decode runs before a
+// CTA's first loads are issued: three hardware divisions there are ~120 instructions in a dependent chain.
+static void set_fast_div(uint32_t out[2], long long d) {
+  out[0] = 0;
+  out[1] = 0;
+  if (d <= 1) return;  // mul = 0: the kernel takes n itself
+  int lg = 0;
+  while ((1ll << lg) < d) ++lg;
+  const int p = 31 + lg;
+  out[0] = (uint32_t)((((unsigned long long)1 << p) + (unsigned long long)d - 1) / (unsigned long long)d);
+  out[1] = (uint32_t)(p - 32);
+}
+
 void hrk_replan(hr_solver* s, int share) {
   if (s->p.variant == 1 || s->p.variant == 2) return;
   if (share < 1) share = 1;
@@ -1047,6 +1061,9 @@ void hrk_replan(hr_solver* s, int share) {
     m.nseg = 1;
     m.ncol = (int)((ntiles / slots) * slots);
   }
+  set_fast_div(m.dv_tiles, ntiles);
+  set_fast_div(m.dv_ntx, m.ntx);
+  set_fast_div(m.dv_rem, ntiles * m.nseg - m.ncol);
   const long long items = m.ncol + (ntiles * m.nseg - m.ncol) * m.mseg;
   for (int st = 0; st < 7; ++st) {
     s->march_grid[st] = (int)std::min<long long>(s->march_slots[st], items);

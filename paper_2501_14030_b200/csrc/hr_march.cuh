@@ -163,6 +163,10 @@ struct alignas(64) MarchMaps {
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
   return (uint32_t)__cvta_generic_to_shared(p);
 }
+// n / d for 0 <= n < 2^31 with the multiplier and shift the host derived from d (MarchPlan::dv_*)
+__device__ __forceinline__ int fast_div(int n, const uint32_t dv[2]) {
+  return dv[0] ? (int)(__umulhi((uint32_t)n, dv[0]) >> dv[1]) : n;
+}
 // one lane of a converged warp (the TMA issue then compiles to straight-line uniform-datapath code instead of a
 // loop over the active lanes of a divergent branch)
 __device__ __forceinline__ bool elect_one() {
@@ -640,16 +644,16 @@ __global__ void __launch_bounds__((TW / VX) * BY,
     // chunks of the remaining segments follow one by one, chunk-major, to even out the end of the launch.
     int tile_id, ch0, nch;
     if (item < plan.ncol) {
-      const int sgi = item / ntiles;
+      const int sgi = fast_div(item, plan.dv_tiles);
       tile_id = item - sgi * ntiles;
       ch0 = sgi * plan.mseg;
       nch = min(plan.mseg, plan.nzc - ch0);
     } else {
       const int nrem = n_long - plan.ncol;
       const int rem = item - plan.ncol;
-      const int cpos = rem / nrem;
+      const int cpos = fast_div(rem, plan.dv_rem);
       const int sid = plan.ncol + (rem - cpos * nrem);
-      const int sgi = sid / ntiles;
+      const int sgi = fast_div(sid, plan.dv_tiles);
       tile_id = sid - sgi * ntiles;
       ch0 = sgi * plan.mseg + cpos;
       nch = ch0 < plan.nzc ? 1 : 0;  // the last segment of a tile may be shorter: an empty item
@@ -657,7 +661,7 @@ __global__ void __launch_bounds__((TW / VX) * BY,
     }
     const int zi = ch0 * plan.zc;
     const int seg = nch > 0 ? min(nch * plan.zc, g.n2 - zi) : 0;
-    const int tx = tile_id % plan.ntx, ty = tile_id / plan.ntx;
+    const int ty = fast_div(tile_id, plan.dv_ntx), tx = tile_id - ty * plan.ntx;
     const int z_begin = NG + zi, z_end = z_begin + seg;
     const int x0 = NG + tx * TW, y0 = NG + ty * BY;  // first point of the tile
     const int i0 = x0 + VX * lx, i1 = y0 + ly;
