@@ -595,6 +595,7 @@ hr_status hr_create(const hr_params* p, void* workspace_dev, size_t workspace_by
   }
   s->n_outer = (int64_t)s->outer_idx.size();
   s->g.n_o2 = (int32_t)H.opos.size();
+  hrk_replan(s, 1);  // the plan carries the multiply-shift constants of g.n_o2 (outer-point loop)
   HR_TRY(upload(a.Wvol, H.wv.data(), np * 8, s->stream));
   {
     // device copies of the inner lists in stored (padded) indices; the host copies stay public

@@ -165,6 +165,7 @@ struct MarchPlan {
   // quotients of the work-item decode by multiplication: q = umulhi(n, mul) >> shr for 0 <= n < 2^31 (mul = 0: the
   // divisor is 1 or unused), for the divisors ntx * nty, ntx and ntx * nty * nseg - ncol; set by hrk_replan
   uint32_t dv_tiles[2], dv_ntx[2], dv_rem[2];
+  uint32_t dv_o2[2], dv_T0[2];  // the same for the outer-point loop: by g.n_o2 and g.T0
   int pdl;       // programmatic-launch trigger: 1 = at entry where every CTA has one item, 0 = always after the
                  // item loop (solvers that share the GPU in hr_step_many), 2 = always at entry (HR_TUNE_PDL)
 };

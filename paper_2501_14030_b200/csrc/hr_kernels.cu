@@ -1064,6 +1064,8 @@ void hrk_replan(hr_solver* s, int share) {
   set_fast_div(m.dv_tiles, ntiles);
   set_fast_div(m.dv_ntx, m.ntx);
   set_fast_div(m.dv_rem, ntiles * m.nseg - m.ncol);
+  set_fast_div(m.dv_o2, s->g.n_o2);
+  set_fast_div(m.dv_T0, s->g.T0);
   const long long items = m.ncol + (ntiles * m.nseg - m.ncol) * m.mseg;
   for (int st = 0; st < 7; ++st) {
     s->march_grid[st] = (int)std::min<long long>(s->march_slots[st], items);

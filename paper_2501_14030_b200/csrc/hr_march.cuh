@@ -517,13 +517,13 @@ __global__ void __launch_bounds__((TW / VX) * BY,
         if (m < nzg) {
           const int pz = m / A, q = m - pz * A;
           i2 = pz < NG ? pz : g.n2 + pz;
-          i1 = q / g.T0;
+          i1 = fast_div(q, plan.dv_T0);
           i0 = q - i1 * g.T0;
         } else {
           const int mm2 = m - nzg, pz = mm2 / ring, r = mm2 - pz * ring;
           i2 = NG + pz;
           if (r < 2 * NG * g.T0) {
-            const int pr = r / g.T0;
+            const int pr = fast_div(r, plan.dv_T0);
             i1 = pr < NG ? pr : g.n1 + pr;
             i0 = r - pr * g.T0;
           } else {
@@ -571,14 +571,14 @@ __global__ void __launch_bounds__((TW / VX) * BY,
         ku = -cw * (au + uc * ir);
         kv = -cw * (av + vc * ir);
       } else {
-        const int qo = m % g.n_o2;
-        i2 = NG + m / g.n_o2;
+        const int pz = fast_div(m, plan.dv_o2), qo = m - pz * g.n_o2;
+        i2 = NG + pz;
         const T r0 = a.RAD0[qo], r1 = a.RAD1[qo], ri = a.RADI[qo];
         if (plan.cyl) {  // C24: the list of outer positions of the plane with their stencil bits
           const int po = a.OPOS[qo];
           const int q = po & 0x0fffffff;
           const int bits = po >> 28;
-          i1 = q / g.T0;
+          i1 = fast_div(q, plan.dv_T0);
           i0 = q - i1 * g.T0;
           c = g.off0 + i0 + g.P0 * i1 + s2 * i2;
           uc = a.in_u[c];
