@@ -508,6 +508,40 @@ def test_work_item_order_knobs_do_not_change_results(hr, monkeypatch):
                     assert np.array_equal(a, b)
 
 
+def test_programmatic_launch_trigger_placement_changes_nothing(hr, monkeypatch):
+    """HR_TUNE_PDL moves griddepcontrol.launch_dependents (never early / early where every CTA has one item / always at
+    entry): the next substep may only START earlier, it reads nothing before its predecessor has completed, so the
+    state after some steps and the fused residual are bit for bit the same -- on a grid with one item per CTA
+    (config 0), one with items handed out dynamically (70 x 1200 x 14, long items) and through hr_step_many."""
+    import torch
+    for params in (W.config(0), W.sweep_point(7, (70, 1200, 14), "SinhSymTP", 6)):
+        for dtype in ("f64", "f32"):
+            ref = None
+            for pdl in (None, "0", "1", "2"):
+                if pdl is None:
+                    monkeypatch.delenv("HR_TUNE_PDL", raising=False)
+                else:
+                    monkeypatch.setenv("HR_TUNE_PDL", pdl)
+                s, t = hr.Solver(params, dtype=dtype), hr.Solver(params, dtype=dtype)
+                out = torch.zeros(2, dtype=torch.float64, device="cuda")
+                for _ in range(6):
+                    s.hr_step_residual_async(0, out)
+                s.hr_step(5)
+                hr.hr_step_many([t], 11)
+                s.synchronize()
+                got = (s.hr_get_u(), s.hr_get_v(), out.cpu().numpy(), t.hr_get_u())
+                s.close()
+                t.close()
+                assert np.array_equal(got[0], got[3])
+                if ref is None:
+                    ref = got
+                    assert np.all(np.isfinite(got[2])) and got[2][0] > 0.0
+                else:
+                    for a, b in zip(got, ref):
+                        assert np.array_equal(a, b), (params["n"], dtype, pdl)
+    monkeypatch.delenv("HR_TUNE_PDL", raising=False)
+
+
 @pytest.mark.parametrize("name,params", [SMALL[0], SMALL[5], SMALL[4], SMALL[3]],
                          ids=[SMALL[0][0], SMALL[5][0], SMALL[4][0], SMALL[3][0]])
 def test_poisoned_workspace_changes_nothing(hr, name, params):
