@@ -410,6 +410,36 @@ def load_traffic(dtype):
         return None
 
 
+def run_many(args, name):
+    """N independent grids on one GPU (the paper's Fig. 6 shape): hr_step_many = one CUDA graph with a branch per
+    solver.  Host wall clock around `--steps` steps with a device synchronise on both sides (the call is host-driven:
+    one graph replay per 8 steps), after `--warmup` x 8 steps; N = 1 is the sequential reference of the same call."""
+    import torch
+    import paper_2501_14030_b200 as hr
+    out = {"metric": METRIC + ", N independent grids advanced together (hr_step_many)", "unit": UNIT,
+           "n_solvers": args.many, "steps": args.steps, "config": {"workload": name}, "data": "synthetic"}
+    for dtype in ("f64", "f32"):
+        res = {}
+        for n in sorted({1, args.many}):
+            idx = int(name[5:].split(":")[0]) if name.startswith("sweep") else 0
+            ps = [workload(name.replace(f"sweep{idx}", f"sweep{idx + i}", 1)) if name.startswith("sweep") else workload(name)
+                  for i in range(n)]
+            ss = [hr.Solver(q, dtype=dtype) for q in ps]
+            hr.hr_step_many(ss, 8 * args.warmup)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            hr.hr_step_many(ss, args.steps)
+            torch.cuda.synchronize()
+            sec = time.perf_counter() - t0
+            pts = ps[0]["n"][0] * ps[0]["n"][1] * ps[0]["n"][2]
+            res[n] = {"us_per_grid_step": sec / args.steps / n * 1e6, "value": 4.0 * pts * n * args.steps / sec}
+            for x in ss:
+                x.close()
+        out[dtype] = dict(res[args.many], vs_sequential=res[1]["us_per_grid_step"] / res[args.many]["us_per_grid_step"],
+                          sequential_us_per_grid_step=res[1]["us_per_grid_step"])
+    print(json.dumps(out))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -423,11 +453,17 @@ def main():
     ap.add_argument("--no-also", action="store_true", help="skip the extra config0/1/2 timings")
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"],
                     help="precision of the headline leg (f32: for profiling the fp32 kernels alone)")
+    ap.add_argument("--many", type=int, default=0, metavar="N",
+                    help="row f2 instead of the headline line: N independent solvers of --workload advanced together by "
+                         "hr_step_many (PAPER.md:337-347), --steps steps, both precisions; prints its own JSON line")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
     name = args.workload
     p = workload(name)
+    if args.many > 0:
+        run_many(args, name)
+        return
 
     if args.oracle_single:
         oracle_single(p, name)
